@@ -1,0 +1,309 @@
+"""Oracle steps O6-O8: sums, estimates and errors, Vegas.
+
+What the paper fixes: each integrand yields a value and an error estimate
+"produced by the integrator"; per-order totals are sums of the values and the
+errors are combined "using the mean-square norm ... treat this number as the
+delta value (standard deviation)".  Vegas (Cuba) is the default
+integrator.  The estimators and Vegas internals are not in the
+paper; they are DESIGN.md readings R5-R8, restated here step by step.
+
+A sector is described by plain data (no CUDA-path types):
+    SectorSpec(texts=[K expression blocks], sector_id, is_complex,
+               deform_f_index, lam)
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+
+import numpy as np
+
+from . import points as P
+from .deform import evaluate_deformed
+from .evaluate import evaluate, LD, CLD
+from .parser import parse
+
+U64 = np.uint64
+
+
+@dataclass
+class SectorSpec:
+    texts: list                 # K expression blocks in the paper's grammar
+    sector_id: int = 0
+    is_complex: bool = False    # PAPER.md:477 (-complex)
+    deform_f_index: int = 0     # >=1: f[deform_f_index] is the polynomial F of the deformation
+    lam: float = 0.0
+    progs: list = field(default_factory=list)
+
+    def __post_init__(self):
+        if not self.progs:
+            self.progs = [parse(t) for t in self.texts]
+        self.dim = self.progs[0].nvars
+        self.K = len(self.progs)
+
+
+def neumaier_sum(values):
+    """Compensated sum of a 1-D long-double array in index order (O6)."""
+    s = values.dtype.type(0)
+    c = values.dtype.type(0)
+    for v in values:
+        t = s + v
+        if abs(s) >= abs(v):
+            c += (s - t) + v
+        else:
+            c += (v - t) + s
+        s = t
+    return s + c
+
+
+def integrand_values(sec: SectorSpec, x, xbar=None, rdtype=LD):
+    """o_k at the points, shape [K, npts]; complex dtype if the sector is complex.
+
+    With deformation every x becomes z(x) and the result is multiplied by det J (R11).
+    The lattice / Vegas weight W is NOT included.
+    """
+    cdtype = CLD if rdtype == LD else np.complex128
+    out = []
+    for prog in sec.progs:
+        if sec.deform_f_index > 0:
+            out.append(evaluate_deformed(prog, sec.deform_f_index, sec.lam, x, xbar, rdtype))
+        elif sec.is_complex:
+            out.append(evaluate(prog, np.asarray(x, dtype=rdtype).astype(cdtype), cdtype))
+        else:
+            out.append(evaluate(prog, x, rdtype))
+    return np.stack(out)
+
+
+def _components(g):
+    """Real sectors: [g]; complex: [Re g, Im g] (each its own estimate, R5)."""
+    return [g.real, g.imag] if np.iscomplexobj(g) else [g]
+
+
+def lattice_points(sec: SectorSpec, n_lattice, genvec, r_periodize, seed, shift_index, first, count, rdtype=LD):
+    """x, xbar, W (product of w_r) of lattice points j = first..first+count-1 of one shift."""
+    j = np.arange(first, first + count, dtype=U64)
+    delta = P.lattice_shift(seed, sec.sector_id, shift_index, sec.dim)
+    t = P.lattice_t(j, genvec, n_lattice, delta)
+    u = P.unit_from_t(t, rdtype)
+    x, xbar, w = P.korobov_transform(u, r_periodize)
+    return x, xbar, np.prod(w, axis=1)
+
+
+def lattice_partial_sums(sec: SectorSpec, n_lattice, n_shifts, genvec, r_periodize, seed, chunk=1 << 14, rdtype=LD):
+    """S1[r,k,c] = sum_j g, S2[r,k,c] = sum_j g^2, SA[r,k,c] = sum_j |g|, g = W*o_k component c.
+
+    Shapes [R, K, C], C = 1 (real) or 2 (Re, Im).  Sums run in index order over j (O6).
+    """
+    ncomp = 2 if (sec.is_complex or sec.deform_f_index > 0) else 1
+    s1 = np.zeros((n_shifts, sec.K, ncomp), dtype=rdtype)
+    s2 = np.zeros_like(s1)
+    sa = np.zeros_like(s1)
+    for r in range(n_shifts):
+        parts = [[[[], [], []] for _ in range(ncomp)] for _ in range(sec.K)]
+        for first in range(0, n_lattice, chunk):
+            cnt = min(chunk, n_lattice - first)
+            x, xbar, w = lattice_points(sec, n_lattice, genvec, r_periodize, seed, r, first, cnt, rdtype)
+            vals = integrand_values(sec, x, xbar, rdtype)
+            for k in range(sec.K):
+                for c, comp in enumerate(_components(vals[k])):
+                    g = w * comp
+                    parts[k][c][0].append(np.sum(g))
+                    parts[k][c][1].append(np.sum(g * g))
+                    parts[k][c][2].append(np.sum(np.abs(g)))
+        for k in range(sec.K):
+            for c in range(ncomp):
+                s1[r, k, c] = neumaier_sum(np.array(parts[k][c][0], dtype=rdtype))
+                s2[r, k, c] = neumaier_sum(np.array(parts[k][c][1], dtype=rdtype))
+                sa[r, k, c] = neumaier_sum(np.array(parts[k][c][2], dtype=rdtype))
+    return s1, s2, sa
+
+
+def estimate_from_sums(s1, s2, n_per_shift):
+    """(value, sigma) from per-shift sums (R5).
+
+    R >= 2 shifts:  Q_r = S1_r/N_L, value = mean_r Q_r,
+                    sigma = sqrt( sum_r (Q_r - value)^2 / (R (R-1)) ).
+    R == 1 (or plain MC): value = <g>, sigma = sqrt( (<g^2> - <g>^2) / (N-1) ), clamped at 0.
+    Leading axis of s1, s2 is the shift index.
+    """
+    dt = s1.dtype.type
+    nshift = s1.shape[0]
+    q = s1 / dt(n_per_shift)
+    if nshift >= 2:
+        value = np.sum(q, axis=0) / dt(nshift)
+        var = np.sum((q - value) ** 2, axis=0) / dt(nshift * (nshift - 1))
+    else:
+        value = q[0]
+        var = (s2[0] / dt(n_per_shift) - value * value) / dt(n_per_shift - 1)
+    return value, np.sqrt(np.maximum(var, 0))
+
+
+def integrate_lattice(sec: SectorSpec, npoints, n_shifts, genvec, r_periodize, seed, chunk=1 << 14, rdtype=LD):
+    """value[K,C], sigma[K,C] of one sector; npoints = R * N_L total (R6)."""
+    n_lattice = npoints // n_shifts
+    s1, s2, _ = lattice_partial_sums(sec, n_lattice, n_shifts, genvec, r_periodize, seed, chunk, rdtype)
+    return estimate_from_sums(s1, s2, n_lattice)
+
+
+def mc_points(sec: SectorSpec, seed, iteration, first, count, rdtype=LD):
+    """y[j,:] uniform in the cube from the Philox MC stream (R3), as (t integers, y)."""
+    j = np.arange(first, first + count, dtype=U64)
+    t = P.philox_t(seed, sec.sector_id, P.TAG_MC, iteration, j, sec.dim)
+    return t, P.unit_from_t(t, rdtype)
+
+
+def integrate_mc(sec: SectorSpec, npoints, seed, chunk=1 << 14, rdtype=LD):
+    """Plain Monte Carlo: x = u, W = 1; value, sigma per (order, component) (R5)."""
+    ncomp = 2 if (sec.is_complex or sec.deform_f_index > 0) else 1
+    p1 = [[[] for _ in range(ncomp)] for _ in range(sec.K)]
+    p2 = [[[] for _ in range(ncomp)] for _ in range(sec.K)]
+    for first in range(0, npoints, chunk):
+        cnt = min(chunk, npoints - first)
+        _, y = mc_points(sec, seed, 0, first, cnt, rdtype)
+        vals = integrand_values(sec, y, None, rdtype)
+        for k in range(sec.K):
+            for c, comp in enumerate(_components(vals[k])):
+                p1[k][c].append(np.sum(comp))
+                p2[k][c].append(np.sum(comp * comp))
+    s1 = np.array([[neumaier_sum(np.array(p1[k][c], dtype=rdtype)) for c in range(ncomp)] for k in range(sec.K)], dtype=rdtype)
+    s2 = np.array([[neumaier_sum(np.array(p2[k][c], dtype=rdtype)) for c in range(ncomp)] for k in range(sec.K)], dtype=rdtype)
+    return estimate_from_sums(s1[None], s2[None], npoints)
+
+
+# ----------------------------------------------------------------------------- Vegas (R8)
+
+def vegas_uniform_grid(dim, nbins, rdtype=LD):
+    return np.tile(np.arange(nbins + 1, dtype=rdtype) / rdtype(nbins), (dim, 1))
+
+
+def vegas_bin_and_frac(t, nbins, rdtype=LD):
+    """b = floor(y*NB) and frac = y*NB - b with y = (2s+1)/2^53, s = t>>12: exact integers (R8)."""
+    s = np.asarray(t, dtype=U64) >> U64(12)
+    prod = (U64(2) * s + U64(1)) * U64(nbins)   # < 2^53 * NB < 2^64 for NB < 2048
+    b = (prod >> U64(53)).astype(np.int64)
+    rem = prod & U64((1 << 53) - 1)
+    return b, rem.astype(rdtype) * rdtype(2.0 ** -53)
+
+
+def vegas_map(t, grid, rdtype=LD):
+    """x[j,d] = xi_b + frac*(xi_{b+1}-xi_b), W[j] = prod_d NB*(xi_{b+1}-xi_b), bins b[j,d]."""
+    dim, nb1 = grid.shape
+    nbins = nb1 - 1
+    b, frac = vegas_bin_and_frac(t, nbins, rdtype)
+    x = np.empty(b.shape, dtype=rdtype)
+    w = np.ones(b.shape[0], dtype=rdtype)
+    for d in range(dim):
+        lo = grid[d][b[:, d]]
+        width = grid[d][b[:, d] + 1] - lo
+        x[:, d] = lo + frac[:, d] * width
+        w = w * (rdtype(nbins) * width)
+    return x, w, b
+
+
+def vegas_refine(grid_d, hist_d, alpha):
+    """New edges of one dimension from its histogram (R8, sub-steps i-iv)."""
+    dt = grid_d.dtype.type
+    nb = hist_d.shape[0]
+    h = hist_d
+    # (i) smooth
+    sm = np.empty_like(h)
+    sm[0] = (h[0] + h[1]) / dt(2)
+    sm[-1] = (h[-2] + h[-1]) / dt(2)
+    sm[1:-1] = (h[:-2] + h[1:-1] + h[2:]) / dt(3)
+    tot = np.sum(sm)
+    if not tot > 0:
+        return grid_d.copy()
+    # (ii) normalise
+    p = sm / tot
+    # (iii) compress
+    m = np.zeros_like(p)
+    mid = (p > 0) & (p < 1)
+    with np.errstate(all="ignore"):
+        m[mid] = ((dt(1) - p[mid]) / (-np.log(p[mid]))) ** dt(alpha)
+    m[p >= 1] = dt(1)
+    # (iv) re-bin: equal sum(m)/NB in every new bin, linear interpolation inside old bins
+    cum = np.zeros(nb + 1, dtype=grid_d.dtype)
+    for b in range(nb):
+        cum[b + 1] = cum[b] + m[b]
+    new = np.empty_like(grid_d)
+    new[0] = dt(0)
+    new[nb] = dt(1)
+    for i in range(1, nb):
+        target = dt(i) * cum[nb] / dt(nb)
+        k = int(np.sum(cum[1:nb] <= target))      # cum[k] <= target < cum[k+1]
+        new[i] = grid_d[k] + (target - cum[k]) / m[k] * (grid_d[k + 1] - grid_d[k])
+    return new
+
+
+def vegas_iteration_sums(sec: SectorSpec, grid, npoints, seed, iteration, chunk=1 << 14, rdtype=LD):
+    """S1[K,C], S2[K,C] and histogram h[dim, NB] (sum over orders/components of g^2) of one iteration."""
+    ncomp = 2 if (sec.is_complex or sec.deform_f_index > 0) else 1
+    nbins = grid.shape[1] - 1
+    p1 = [[[] for _ in range(ncomp)] for _ in range(sec.K)]
+    p2 = [[[] for _ in range(ncomp)] for _ in range(sec.K)]
+    hist = np.zeros((sec.dim, nbins), dtype=rdtype)
+    for first in range(0, npoints, chunk):
+        cnt = min(chunk, npoints - first)
+        t, _ = mc_points(sec, seed, iteration, first, cnt, rdtype)
+        x, w, b = vegas_map(t, grid, rdtype)
+        vals = integrand_values(sec, x, None, rdtype)
+        g2 = np.zeros(cnt, dtype=rdtype)
+        for k in range(sec.K):
+            for c, comp in enumerate(_components(vals[k])):
+                g = w * comp
+                p1[k][c].append(np.sum(g))
+                p2[k][c].append(np.sum(g * g))
+                g2 = g2 + g * g
+        for d in range(sec.dim):
+            np.add.at(hist[d], b[:, d], g2)      # h[d][b] += g^2, one point after another
+    s1 = np.array([[neumaier_sum(np.array(p1[k][c], dtype=rdtype)) for c in range(ncomp)] for k in range(sec.K)], dtype=rdtype)
+    s2 = np.array([[neumaier_sum(np.array(p2[k][c], dtype=rdtype)) for c in range(ncomp)] for k in range(sec.K)], dtype=rdtype)
+    return s1, s2, hist
+
+
+def vegas_combine(i_it, var_it):
+    """Weighted average over iterations, sigma, chi2 (R8).  Arrays [iters, ...]."""
+    dt = i_it.dtype.type
+    var = np.maximum(var_it, 0)
+    pos = var > 0
+    value = np.empty(i_it.shape[1:], dtype=i_it.dtype)
+    sigma = np.empty_like(value)
+    chi2 = np.empty_like(value)
+    for idx in np.ndindex(value.shape):
+        v = var[(slice(None),) + idx]
+        i = i_it[(slice(None),) + idx]
+        if not np.any(v > 0):
+            value[idx], sigma[idx], chi2[idx] = np.sum(i) / dt(len(i)), dt(0), dt(0)
+            continue
+        v = np.where(v > 0, v, np.min(v[v > 0]))
+        wgt = dt(1) / v
+        value[idx] = np.sum(i * wgt) / np.sum(wgt)
+        sigma[idx] = dt(1) / np.sqrt(np.sum(wgt))
+        chi2[idx] = np.sum((i - value[idx]) ** 2 * wgt)
+    return value, sigma, chi2
+
+
+def integrate_vegas(sec: SectorSpec, npoints_per_iter, seed, nbins=50, iters=10, alpha=1.5, chunk=1 << 14,
+                    rdtype=LD, trace=None):
+    """Classic Lepage Vegas as restated in DESIGN.md R8.  Returns value, sigma, chi2 [K,C], final grid.
+
+    `trace`, if a list, receives per iteration a dict(grid=, s1=, s2=, hist=, I=, var=).
+    """
+    grid = vegas_uniform_grid(sec.dim, nbins, rdtype)
+    n = rdtype(npoints_per_iter)
+    i_list, v_list = [], []
+    for it in range(iters):
+        s1, s2, hist = vegas_iteration_sums(sec, grid, npoints_per_iter, seed, it, chunk, rdtype)
+        i_it = s1 / n
+        var_it = (s2 / n - i_it * i_it) / (n - rdtype(1))
+        i_list.append(i_it)
+        v_list.append(var_it)
+        if trace is not None:
+            trace.append(dict(grid=grid.copy(), s1=s1, s2=s2, hist=hist.copy(), I=i_it, var=var_it))
+        grid = np.stack([vegas_refine(grid[d], hist[d], alpha) for d in range(sec.dim)])
+    value, sigma, chi2 = vegas_combine(np.stack(i_list), np.stack(v_list))
+    return value, sigma, chi2, grid
+
+
+def combine_sectors(values, sigmas):
+    """Sum over sectors (leading axis): sum of values, sqrt of the sum of sigma^2."""
+    return np.sum(values, axis=0), np.sqrt(np.sum(np.asarray(sigmas) ** 2, axis=0))

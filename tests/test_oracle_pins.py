@@ -1,0 +1,555 @@
+"""Pins of the oracle against things other than itself: the paper's worked example, closed
+forms, library routines (mpmath, scipy, numpy.linalg, cuRAND host), brute force.  CPU only."""
+import ctypes
+import itertools
+import math
+import os
+
+import mpmath
+import numpy as np
+import pytest
+import scipy.special
+
+from conftest import golden
+from oracle import points as P
+from oracle.deform import (deform, det_lu, differentiate, evaluate_deformed, f_polynomial_tree,
+                           gradient_and_hessian)
+from oracle.evaluate import CLD, LD, evaluate, evaluate_with_magnitude, polygamma_const, PI, EULER_GAMMA
+from oracle.integrate import (SectorSpec, combine_sectors, estimate_from_sums, integrate_lattice, integrate_mc,
+                              integrate_vegas, lattice_partial_sums, neumaier_sum, vegas_combine, vegas_refine,
+                              vegas_uniform_grid)
+from oracle.parser import ParseError, parse
+from workloads import korobov_a
+
+mpmath.mp.dps = 40
+SEED = 20151111
+
+
+def block(nvars, flines, final):
+    return "\n".join([f"{nvars};", f"{len(flines)};"] + [f + ";" for f in flines] + [final + ";", "|"])
+
+
+# ------------------------------------------------------------------ parser + walker
+
+def test_paper_worked_example_integrates_to_0p7():
+    g = golden("paper_worker_example.txt")
+    sec = SectorSpec([g["text"] + "\n|"])
+    n = 1 << 12
+    val, err = integrate_lattice(sec, 8 * n, 8, P.korobov_genvec(korobov_a(n, 1), n, 1), 3, SEED)
+    assert abs(float(val[0, 0]) - float(g["value"])) < 1e-12
+    assert float(err[0, 0]) < 1e-10
+    val, err = integrate_mc(sec, 1 << 14, SEED)
+    assert abs(float(val[0, 0]) - 0.7) < 4 * float(err[0, 0])
+    assert 0 < float(err[0, 0]) < 0.01      # sigma of x+0.2 is sqrt(1/12)/sqrt(N) = 2.3e-3
+
+
+def test_linear_function_closed_form():
+    # "-test: integrator test on a sample linear function": c0 + sum c_k/2
+    rng = np.random.default_rng(1)
+    n = 5
+    c = [float(v) for v in rng.uniform(-2, 2, size=n + 1)]
+    text = block(n, [], "+".join([f"({c[0]!r})"] + [f"({c[k + 1]!r})*x[{k + 1}]" for k in range(n)]))
+    exact = c[0] + sum(c[1:]) / 2
+    nl = 1 << 11
+    val, err = integrate_lattice(SectorSpec([text]), 8 * nl, 8, P.korobov_genvec(korobov_a(nl, 4), nl, n), 3, SEED)
+    assert abs(float(val[0, 0]) - exact) <= max(4 * float(err[0, 0]), 1e-13)
+    assert float(err[0, 0]) < 5e-3
+
+
+def test_walker_against_python_floats():
+    # brute force: the same formula typed as a Python expression, evaluated with math.*
+    text = block(3, ["x[1]*x[2]+0.5", "l[f[1]]-x[3]/(1+x[2])"],
+                 "-f[2]*p[f[1],3]+p[x[3],-2]/f[1]-p[f[1],0.5]*(x[1]-2*x[2])*P+G-(-x[1])")
+    prog = parse(text)
+    rng = np.random.default_rng(2)
+    x = rng.uniform(0.1, 0.9, size=(50, 3))
+    got = evaluate(prog, x, LD)
+    for j in range(50):
+        a, b, c = x[j]
+        f1 = a * b + 0.5
+        f2 = math.log(f1) - c / (1 + b)
+        ref = -f2 * f1 ** 3 + c ** -2 / f1 - f1 ** 0.5 * (a - 2 * b) * math.pi + 0.5772156649015329 - (-a)
+        assert abs(float(got[j]) - ref) <= 2e-15 * max(1.0, abs(ref)) * 20
+
+
+def test_operator_precedence_and_associativity():
+    prog = parse(block(2, [], "1-x[1]-x[2]*2/4/x[1]+-x[2]"))
+    x = np.array([[0.5, 0.25]])
+    assert float(evaluate(prog, x)[0]) == 1 - 0.5 - 0.25 * 2 / 4 / 0.5 + -0.25
+
+
+def test_integer_power_is_repeated_multiplication_and_negative_is_reciprocal():
+    x = np.array([[LD(3) / LD(7)]], dtype=LD)
+    v = x[0, 0]
+    assert evaluate(parse(block(1, [], "p[x[1],4]")), x)[0] == v * v * v * v
+    assert evaluate(parse(block(1, [], "p[x[1],-3]")), x)[0] == 1 / (v * v * v)
+    assert evaluate(parse(block(1, [], "p[x[1],0]")), x)[0] == 1
+    got = evaluate(parse(block(1, [], "p[x[1],-0.7]")), x)[0]
+    # the literal -0.7 denotes its nearest FP64 value ("doubles")
+    assert abs(got - LD(str(mpmath.power(mpmath.mpf(3) / 7, mpmath.mpf(-0.7))))) < 4e-19 * 2
+
+
+def test_real_mode_domain_errors_give_nan():
+    x = np.array([[0.25]])
+    assert np.isnan(evaluate(parse(block(1, [], "l[x[1]-1]")), x)[0])
+    assert np.isnan(evaluate(parse(block(1, [], "p[x[1]-1,0.5]")), x)[0])
+
+
+def test_complex_mode_principal_branches():
+    z = np.array([[-0.3 - 1e-3j]], dtype=CLD)
+    v = evaluate(parse(block(1, [], "l[x[1]]")), z, CLD)[0]
+    ref = mpmath.log(mpmath.mpc(-0.3, -1e-3))
+    assert abs(complex(v) - complex(ref)) < 1e-15 and v.imag < -3.1
+    v = evaluate(parse(block(1, [], "p[x[1],-2.5]")), z, CLD)[0]
+    ref = mpmath.power(mpmath.mpc(-0.3, -1e-3), -2.5)
+    assert abs(complex(v) - complex(ref)) < 1e-13 * abs(complex(ref))
+
+
+def test_constants_against_mpmath():
+    assert abs(PI - LD(str(mpmath.pi))) < 2e-19
+    assert abs(EULER_GAMMA - LD(str(mpmath.euler))) < 1e-19
+    for n, m in ((1, 1), (2, 1), (2, 2), (2, 3), (2, 4), (3, 1), (3, 2)):
+        ref = mpmath.polygamma(n, m)
+        got = polygamma_const(n, m)
+        assert abs(got - LD(str(ref))) < 2e-18 * abs(float(ref)), (n, m)
+        assert abs(float(evaluate(parse(block(1, [], f"PolyGamma[{n},{m}]+0*x[1]")), np.array([[0.5]]))[0])
+                   - float(ref)) < 1e-15 * abs(float(ref))
+
+
+@pytest.mark.parametrize("bad", [
+    "1; 0; x[2];\n|",             # variable out of range
+    "1; 1; f[1]; x[1];\n|",       # f used before defined
+    "1; 0; x[1]+;\n|",
+    "1; 0; PolyGamma[5,5];\n|",   # not hard-coded
+    "1; 2; x[1]; x[1];\n|",       # wrong number of lines
+    "1; 0; x[1]",                 # missing ';'
+    "1; 0; p[x[1],x[1]];\n|",     # exponent must be numeric
+])
+def test_parse_errors(bad):
+    with pytest.raises(ParseError):
+        parse(bad)
+
+
+# ------------------------------------------------------------------ closed forms
+
+def _genvec(nl, dim):
+    return P.korobov_genvec(korobov_a(nl, dim), nl, dim)
+
+
+def test_monomial_integrals_closed_form():
+    # int prod x_i^a_i = prod 1/(a_i+1) over the unit cube (BASELINE config 1's closed-form check)
+    nl = 1 << 13
+    for a in [(0, 1, 2, 1), (2, 2, 0, 1), (-0.45, 1, 0, -0.3)]:
+        text = block(4, [], "*".join(f"p[x[{i + 1}],{ai}]" for i, ai in enumerate(a)))
+        exact = np.prod([1.0 / (ai + 1) for ai in a])
+        val, err = integrate_lattice(SectorSpec([text]), 8 * nl, 8, _genvec(nl, 4), 3, SEED)
+        assert abs(float(val[0, 0]) - exact) <= 4 * float(err[0, 0]) + 1e-15, a
+        assert float(err[0, 0]) < 2e-4 * exact, a
+
+
+def test_bubble_golden_against_mpmath():
+    g = golden("bubble_eps_coefficients.txt")
+    eps = mpmath.mpf(0)
+    coeffs = mpmath.taylor(lambda e: mpmath.gamma(1 - e) ** 2 / mpmath.gamma(2 - 2 * e), eps, 4)
+    for k in range(5):
+        assert abs(coeffs[k] - mpmath.mpf(g[f"c{k}"])) < mpmath.mpf("1e-15")
+
+
+def test_bubble_epsilon_orders():
+    # U = 1 + x1 = f[1], F = x1; order-k integrand (1+t)^-2 (2 ln(1+t) - ln t)^k / k!
+    g = golden("bubble_eps_coefficients.txt")
+    nl = 1 << 13
+    texts = []
+    for k in range(5):
+        fac = math.factorial(k)
+        body = "p[f[1],-2]" + (f"*p[2*l[f[1]]-l[x[1]],{k}]/{fac}" if k else "")
+        texts.append(block(1, ["1+x[1]"], body))
+    val, err = integrate_lattice(SectorSpec(texts), 8 * nl, 8, _genvec(nl, 1), 3, SEED)
+    for k in range(5):
+        exact = float(g[f"c{k}"])
+        assert abs(2 * float(val[k, 0]) - exact) <= 2 * 4 * float(err[k, 0]) + 1e-14, k
+        assert abs(2 * float(val[k, 0]) - exact) < 1e-9, k
+
+
+def test_random_family_against_gauss_legendre_bruteforce():
+    # 2-D U^p / F^q * log with random coefficients; reference = tensor Gauss-Legendre on the Python formula
+    rng = np.random.default_rng(5)
+    cu, cf = [float(v) for v in rng.uniform(0.5, 2, 4)], [float(v) for v in rng.uniform(0.5, 2, 4)]
+    texts = [block(2, [f"{cu[0]!r}+{cu[1]!r}*x[1]+{cu[2]!r}*x[1]*x[2]+{cu[3]!r}*p[x[2],2]",
+                       f"{cf[0]!r}+{cf[1]!r}*x[2]+{cf[2]!r}*x[1]*x[2]+{cf[3]!r}*p[x[1],2]"],
+                   "x[1]*f[1]*p[f[2],-2.5]*l[f[2]]")]
+    xs, ws = np.polynomial.legendre.leggauss(60)
+    xs, ws = (xs + 1) / 2, ws / 2
+    X, Y = np.meshgrid(xs, xs, indexing="ij")
+    U = cu[0] + cu[1] * X + cu[2] * X * Y + cu[3] * Y ** 2
+    F = cf[0] + cf[1] * Y + cf[2] * X * Y + cf[3] * X ** 2
+    ref = float(np.sum(np.outer(ws, ws) * X * U * F ** -2.5 * np.log(F)))
+    nl = 1 << 13
+    val, err = integrate_lattice(SectorSpec(texts), 8 * nl, 8, _genvec(nl, 2), 3, SEED)
+    assert abs(float(val[0, 0]) - ref) <= 4 * float(err[0, 0]) + 1e-12
+    assert abs(float(val[0, 0]) - ref) < 1e-8 * abs(ref)
+
+
+# ------------------------------------------------------------------ points
+
+def test_lattice_integers_against_bigint_bruteforce():
+    nl, dim, a = 1 << 9, 5, 187
+    g = P.korobov_genvec(a, nl, dim)
+    assert g == [pow(a, k, nl) for k in range(dim)]
+    delta = P.lattice_shift(SEED, 7, 3, dim)
+    t = P.lattice_t(np.arange(nl), g, nl, delta)
+    for j in (0, 1, 2, 255, 511):
+        for k in range(dim):
+            ref = ((((j * g[k]) % nl) << 64) // nl + int(delta[k])) % (1 << 64)
+            assert int(t[j, k]) == ref
+    u = P.unit_from_t(t)
+    for j in (0, 3, 400):
+        for k in range(dim):
+            assert u[j, k] == LD(2 * (int(t[j, k]) >> 12) + 1) / LD(2 ** 53)
+    assert np.all((u > 0) & (u < 1))
+    assert np.all(u.astype(np.float64).astype(LD) == u)      # exactly representable in FP64
+
+
+def test_lattice_character_sums_vanish():
+    # (1/N) sum_j exp(2 pi i h.(j g + Delta)/N) = 0 unless h.g = 0 mod N: exactness of the rank-1 rule
+    nl, dim = 1 << 10, 3
+    g = P.korobov_genvec(korobov_a(nl, dim), nl, dim)
+    t = P.lattice_t(np.arange(nl), g, nl, P.lattice_shift(SEED, 0, 0, dim)).astype(LD) / LD(2) ** 64
+    rng = np.random.default_rng(3)
+    n_zero = 0
+    for _ in range(40):
+        h = rng.integers(-6, 7, size=dim)
+        s = np.sum(np.cos(2 * PI * (t @ h.astype(LD)))) / nl
+        if int(np.dot(h, g)) % nl == 0:
+            continue
+        n_zero += 1
+        assert abs(float(s)) < 1e-13
+    assert n_zero > 30
+
+
+def test_philox_against_curand_host_generator():
+    # cuRAND's host generator (a CPU library routine) hands out raw Philox4x32-10 words; group i of four
+    # words is the block with counter (i // T, 0, i % T, 0) and key = seed, T = cuRAND's stream count.
+    path = "/usr/local/cuda/lib64/libcurand.so"
+    if not os.path.exists(path):
+        pytest.skip("cuRAND not installed")
+    lib = ctypes.CDLL(path)
+    ngroups = 70000
+    for seed in (0, SEED, 0xDEADBEEFCAFE1234):
+        gen = ctypes.c_void_p()
+        assert lib.curandCreateGeneratorHost(ctypes.byref(gen), 161) == 0   # CURAND_RNG_PSEUDO_PHILOX4_32_10
+        assert lib.curandSetPseudoRandomGeneratorSeed(gen, ctypes.c_ulonglong(seed)) == 0
+        out = np.zeros(4 * ngroups, dtype=np.uint32)
+        assert lib.curandGenerate(gen, out.ctypes.data_as(ctypes.c_void_p), ctypes.c_size_t(out.size)) == 0
+        lib.curandDestroyGenerator(gen)
+        out = out.reshape(-1, 4).astype(np.uint64)
+        i = np.arange(ngroups)
+        matched = False
+        for log_t in range(10, 21):
+            t = 1 << log_t
+            mine = np.stack(P.philox4x32_10(i // t, 0 * i, i % t, 0 * i, seed & 0xFFFFFFFF, seed >> 32), axis=1)
+            if np.array_equal(mine, out):
+                matched = t < ngroups           # both c0 and c2 varied
+                break
+        assert matched, seed
+
+
+def test_philox_stream_layout_and_moments():
+    t = P.philox_t(SEED, 5, P.TAG_MC, 2, np.arange(4096), 7)
+    # layout (R3): coordinate pair (2kb, 2kb+1) = words (0,1), (2,3) of the call with kblock kb
+    o = P.philox4x32_10([9], [0], [5], [(1 << 28) | (2 << 20) | 2], SEED & 0xFFFFFFFF, SEED >> 32)
+    assert int(t[9, 4]) == (int(o[0][0]) << 32) | int(o[1][0])
+    assert int(t[9, 5]) == (int(o[2][0]) << 32) | int(o[3][0])
+    u = P.unit_from_t(t).astype(np.float64)
+    assert abs(u.mean() - 0.5) < 4 * math.sqrt(1 / 12 / u.size)
+    assert abs((u ** 2).mean() - 1 / 3) < 4 * math.sqrt(4 / 45 / u.size)
+    assert abs(np.corrcoef(u[:, 0], u[:, 1])[0, 1]) < 4 / math.sqrt(4096)
+    assert len(np.unique(t)) == t.size
+    assert not np.array_equal(P.lattice_shift(SEED, 5, 0, 4), P.lattice_shift(SEED, 6, 0, 4))
+    assert not np.array_equal(P.lattice_shift(SEED, 5, 0, 4), P.lattice_shift(SEED, 5, 1, 4))
+
+
+@pytest.mark.parametrize("r", [1, 2, 3, 4])
+def test_korobov_transform_against_incomplete_beta(r):
+    u = np.linspace(0, 1, 1001, dtype=LD)[1:-1]
+    x, xbar, w = P.korobov_transform(u, r)
+    ref = scipy.special.betainc(r + 1, r + 1, u.astype(np.float64))     # phi_r = I_u(r+1, r+1)
+    assert np.max(np.abs(x.astype(np.float64) - ref)) < 5e-15
+    assert np.max(np.abs((x + xbar) - 1)) < 2e-19
+    x2, xbar2, w2 = P.korobov_transform(LD(1) - u, r)
+    assert np.max(np.abs(x2 - xbar)) < 2e-19 and np.max(np.abs(w2 - w)) < 1e-17     # phi(u)+phi(1-u)=1
+    wref = math.factorial(2 * r + 1) / math.factorial(r) ** 2 * (u * (1 - u)) ** r
+    assert np.max(np.abs(w - wref)) < 1e-15
+    # phi' = w (central differences) and int w = 1 (Gauss-Legendre, exact for degree 2r)
+    h = LD(1e-6)
+    d = (P.korobov_transform(u + h, r)[0] - P.korobov_transform(u - h, r)[0]) / (2 * h)
+    assert np.max(np.abs(d - w)) < 1e-9
+    gx, gw = np.polynomial.legendre.leggauss(12)
+    assert abs(float(np.sum(gw / 2 * np.asarray(P.korobov_transform(np.asarray((gx + 1) / 2, dtype=LD), r)[2],
+                                                dtype=np.float64))) - 1) < 1e-14
+    # near the faces: x = phi(u) keeps full relative accuracy, xbar does near u -> 1
+    tiny = np.array([LD(2) ** -40], dtype=LD)
+    xs, _, _ = P.korobov_transform(tiny, r)
+    lead = math.factorial(2 * r + 1) / math.factorial(r) ** 2 / (r + 1)
+    assert abs(float(xs[0]) / (lead * float(tiny[0]) ** (r + 1)) - 1) < 1e-10
+    _, xb, _ = P.korobov_transform(LD(1) - tiny, r)
+    assert xb[0] == xs[0]
+
+
+def test_transformed_singular_integral():
+    # int phi_3(u)^-0.7 w_3(u) du = int x^-0.7 dx = 1/0.3
+    nl = 1 << 13
+    val, err = integrate_lattice(SectorSpec([block(1, [], "p[x[1],-0.7]")]), 8 * nl, 8, _genvec(nl, 1), 3, SEED)
+    assert abs(float(val[0, 0]) - 1 / 0.3) <= 4 * float(err[0, 0]) + 1e-12
+
+
+# ------------------------------------------------------------------ deformation
+
+F_TEXT = "0.7-1.3*x[1]*x[2]+0.9*p[x[3],2]*x[1]-0.4*x[2]+p[x[1]+x[3],3]/4"
+
+
+def test_derivatives_against_complex_step_and_differences():
+    prog = parse(block(3, [F_TEXT], "f[1]"))
+    rng = np.random.default_rng(4)
+    x = rng.uniform(0.05, 0.95, size=(20, 3)).astype(LD)
+    g, h = gradient_and_hessian(prog, 1, x)
+    step = LD("1e-30")
+    for k in range(3):
+        z = x.astype(CLD)
+        z[:, k] += 1j * step
+        cs = evaluate(prog, z, CLD).imag / step                   # Im F(x + i h e_k)/h
+        assert np.max(np.abs(cs - g[:, k])) < 1e-17
+        for l in range(3):
+            d = LD("1e-9")
+            xp, xm = x.copy(), x.copy()
+            xp[:, l] += d
+            xm[:, l] -= d
+            fd = (gradient_and_hessian(prog, 1, xp)[0][:, k] - gradient_and_hessian(prog, 1, xm)[0][:, k]) / (2 * d)
+            assert np.max(np.abs(fd - h[:, k, l])) < 1e-8
+    # hand-derived gradient of F_TEXT
+    a, b, c = (x[:, i] for i in range(3))
+    assert np.max(np.abs(g[:, 0] - (-1.3 * b + 0.9 * c * c + 0.75 * (a + c) ** 2))) < 1e-15
+    assert np.max(np.abs(g[:, 1] - (-1.3 * a - 0.4))) < 1e-15
+    assert np.max(np.abs(h[:, 0, 2] - (1.8 * c + 1.5 * (a + c)))) < 1e-15
+
+
+def test_det_lu_against_cofactors_and_numpy():
+    rng = np.random.default_rng(6)
+    for n in (1, 2, 3, 4):
+        a = (rng.normal(size=(30, n, n)) + 1j * rng.normal(size=(30, n, n))).astype(CLD)
+        ref = np.zeros(30, dtype=CLD)
+        for perm in itertools.permutations(range(n)):                 # Leibniz formula
+            sign = np.linalg.det(np.eye(n)[list(perm)])
+            term = np.full(30, sign, dtype=CLD)
+            for i, p in enumerate(perm):
+                term = term * a[:, i, p]
+            ref += term
+        assert np.max(np.abs(det_lu(a) - ref) / np.abs(ref)) < 1e-15
+    a = (rng.normal(size=(10, 7, 7)) + 1j * rng.normal(size=(10, 7, 7))).astype(CLD)
+    ref = np.linalg.det(a.astype(np.complex128))
+    assert np.max(np.abs(det_lu(a).astype(np.complex128) - ref) / np.abs(ref)) < 1e-12
+    tri = np.triu(a)
+    assert np.max(np.abs(det_lu(tri) - np.prod(np.diagonal(tri, axis1=1, axis2=2), axis=1))) < 1e-16
+    a[:, 0, :] = 0          # singular column pivot must give 0, not NaN-free garbage
+    assert np.all(det_lu(a[:, :, :]) == 0) or np.all(np.isnan(det_lu(a).real))
+
+
+def test_deformation_matches_its_definition_and_jacobian_is_dz_dx():
+    prog = parse(block(3, [F_TEXT], "f[1]"))
+    rng = np.random.default_rng(7)
+    x = rng.uniform(0.05, 0.95, size=(8, 3)).astype(LD)
+    lam = 0.5
+    z, jac = deform(prog, 1, lam, x)
+    g, _ = gradient_and_hessian(prog, 1, x)
+    assert np.max(np.abs(z - (x - 1j * LD(lam) * x * (1 - x) * g))) < 1e-18
+    d = LD("1e-9")
+    for l in range(3):
+        xp, xm = x.copy(), x.copy()
+        xp[:, l] += d
+        xm[:, l] -= d
+        fd = (deform(prog, 1, lam, xp)[0] - deform(prog, 1, lam, xm)[0]) / (2 * d)
+        assert np.max(np.abs(fd - jac[:, :, l])) < 1e-8             # J_kl = dz_k/dx_l
+    z0, j0 = deform(prog, 1, 0.0, x)
+    assert np.all(z0.imag == 0) and np.all(det_lu(j0) == 1)         # lambda = 0 is the real path
+
+
+def test_contour_1d_closed_forms():
+    g = golden("contour_1d_closed_forms.txt")
+    a = mpmath.mpf("0.3")
+    assert abs(mpmath.log((1 - a) / a) - mpmath.mpf(g["inv_re"])) < 1e-17
+    assert abs(2 * mpmath.sqrt(a) - mpmath.mpf(g["rsqrt_im"])) < 1e-17
+    assert abs((1 - a) * mpmath.log(1 - a) + a * mpmath.log(a) - 1 - mpmath.mpf(g["log_re"])) < 1e-17
+    nl = 1 << 13
+    for key, final in (("inv", "1/f[1]"), ("log", "l[f[1]]"), ("rsqrt", "p[f[1],-0.5]")):
+        sec = SectorSpec([block(1, ["x[1]-0.3"], final)], is_complex=True, deform_f_index=1, lam=0.5)
+        val, err = integrate_lattice(sec, 8 * nl, 8, _genvec(nl, 1), 3, SEED)
+        for c, part in enumerate(("re", "im")):
+            exact = float(g[f"{key}_{part}"])
+            assert abs(float(val[0, c]) - exact) <= 4 * float(err[0, c]) + 1e-11, (key, part)
+            assert abs(float(val[0, c]) - exact) < 1e-6, (key, part)
+
+
+def test_lambda_independence_for_entire_integrands():
+    # Cauchy: int g(z) det J dx = int g(x) dx for polynomials g, any lambda, any polynomial F (z fixes the faces)
+    nl = 1 << 12
+    flines = ["0.6-1.1*x[1]*x[2]+0.8*x[3]-0.5*p[x[2],2]*x[3]"]
+    final = "p[x[1],2]*x[2]+0.5*x[3]*x[1]"
+    exact = 1.0 / 6 + 0.125
+    for lam in (0.0, 0.3, 1.0):
+        sec = SectorSpec([block(3, flines, final)], is_complex=True, deform_f_index=1, lam=lam)
+        val, err = integrate_lattice(sec, 8 * nl, 8, _genvec(nl, 3), 3, SEED)
+        assert abs(float(val[0, 0]) - exact) <= 4 * float(err[0, 0]) + 1e-12, lam
+        assert abs(float(val[0, 1])) <= 4 * float(err[0, 1]) + 1e-12, lam
+        assert float(err[0, 0]) < 1e-5
+
+
+def test_c4_workload_has_negative_imaginary_f():
+    # PAPER.md:474 (-testF): "the sign of the imaginary part of F is negative"
+    from workloads import make_workload
+    wl = make_workload("C4", nsectors=3, npoints=1 << 10)
+    rng = np.random.default_rng(8)
+    x = rng.uniform(0, 1, size=(2000, wl.dim)).astype(LD)
+    changes = 0
+    for s in wl.sectors:
+        sec = SectorSpec(s.texts, s.sector_id, True, s.deform_f_index, s.lam)
+        prog = sec.progs[0]
+        z, _ = deform(prog, s.deform_f_index, s.lam, x)
+        from oracle.parser import Program
+        fz = evaluate(Program(prog.nvars, [], f_polynomial_tree(prog, s.deform_f_index)), z, CLD)
+        assert np.all(fz.imag < 0)
+        fx = evaluate(Program(prog.nvars, [], f_polynomial_tree(prog, s.deform_f_index)), x, LD)
+        changes += int(np.any(fx < 0))
+        vals = evaluate_deformed(prog, s.deform_f_index, s.lam, x)
+        assert np.all(np.isfinite(vals.real)) and np.all(np.isfinite(vals.imag))
+
+
+# ------------------------------------------------------------------ estimators
+
+def test_neumaier_and_estimators():
+    v = np.array([LD(1), LD(2) ** -70, -LD(1), LD(2) ** -70], dtype=LD)
+    assert neumaier_sum(v) == LD(2) ** -69
+    # R shifts of a constant integrand: sigma = 0
+    val, err = integrate_lattice(SectorSpec([block(2, [], "2.5+0*x[1]")]), 8 * 64, 8, [1, 19], 0, SEED)
+    assert float(val[0, 0]) == 2.5 and float(err[0, 0]) == 0
+    # R >= 2 formula on hand numbers: Q = (1,2,3,6) -> mean 3, sigma = sqrt(14/12)
+    s1 = np.array([[[10.0]], [[20.0]], [[30.0]], [[60.0]]], dtype=LD)
+    value, sig = estimate_from_sums(s1, s1 * 0, 10)
+    assert float(value[0, 0]) == 3 and abs(float(sig[0, 0]) - math.sqrt(14 / 12)) < 1e-15
+    # R = 1: sqrt((<g^2> - <g>^2)/(N-1)) on g = (1,2,3,4): mean 2.5, <g^2> = 7.5 -> sqrt(1.25/3)
+    value, sig = estimate_from_sums(np.array([[[10.0]]], dtype=LD), np.array([[[30.0]]], dtype=LD), 4)
+    assert float(value[0, 0]) == 2.5 and abs(float(sig[0, 0]) - math.sqrt(1.25 / 3)) < 1e-15
+    # sum the values, errors in mean square
+    tot, sig = combine_sectors(np.array([[1.0, 2.0], [3.0, 4.0]]), np.array([[3.0, 0.0], [4.0, 1.0]]))
+    assert list(tot) == [4.0, 6.0] and list(sig) == [5.0, 1.0]
+
+
+def test_four_sigma_coverage_over_seeds():
+    # the reported error must be an honest standard deviation: R = 8 shifts -> t_7 pulls
+    nl = 1 << 9
+    sec = SectorSpec([block(3, [], "p[x[1],2]*x[2]*p[1+x[3],-1]")])
+    exact = (1 / 3) * (1 / 2) * math.log(2)
+    pulls = []
+    for seed in range(60):
+        val, err = integrate_lattice(sec, 8 * nl, 8, _genvec(nl, 3), 3, seed)
+        pulls.append((float(val[0, 0]) - exact) / float(err[0, 0]))
+    pulls = np.array(pulls)
+    assert np.sum(np.abs(pulls) > 4) <= 2
+    assert 0.6 < np.sqrt(np.mean(pulls ** 2)) < 2.0            # t_7: sqrt(7/5) = 1.18
+
+
+# ------------------------------------------------------------------ Vegas (R8)
+
+def test_vegas_refine_flat_histogram_keeps_uniform_grid():
+    grid = vegas_uniform_grid(1, 50)[0]
+    new = vegas_refine(grid, np.full(50, LD(3.7)), 1.5)
+    assert np.max(np.abs(new - grid)) < 1e-15
+    assert new[0] == 0 and new[-1] == 1
+    assert np.array_equal(vegas_refine(grid, np.zeros(50, dtype=LD), 1.5), grid)      # all-zero: unchanged
+
+
+def test_vegas_refine_invariants_and_equalisation():
+    rng = np.random.default_rng(9)
+    grid = np.sort(np.concatenate([[0, 1], rng.uniform(0, 1, 49)])).astype(LD)
+    hist = rng.uniform(0, 1, 50).astype(LD) ** 4
+    hist[5] = 0
+    new = vegas_refine(grid, hist, 1.5)
+    assert new[0] == 0 and new[-1] == 1 and np.all(np.diff(new) > 0)
+    assert abs(float(np.sum(np.diff(new))) - 1) < 1e-17
+    # each new bin holds sum(m)/NB of the piecewise-constant density m_b/(width_b): brute-force check by
+    # integrating that density over the new bins with fine quadrature in float64
+    sm = np.empty(50)
+    h = hist.astype(np.float64)
+    sm[0], sm[-1] = (h[0] + h[1]) / 2, (h[-2] + h[-1]) / 2
+    sm[1:-1] = (h[:-2] + h[1:-1] + h[2:]) / 3
+    p = sm / sm.sum()
+    m = ((1 - p) / -np.log(p)) ** 1.5
+    dens = m / np.diff(grid.astype(np.float64))
+    edges_old = grid.astype(np.float64)
+
+    def mass(a, b):
+        tot = 0.0
+        for k in range(50):
+            lo, hi = max(a, edges_old[k]), min(b, edges_old[k + 1])
+            if hi > lo:
+                tot += dens[k] * (hi - lo)
+        return tot
+    masses = [mass(float(new[i]), float(new[i + 1])) for i in range(50)]
+    assert np.max(np.abs(np.array(masses) - m.sum() / 50)) < 1e-12
+
+
+def test_vegas_constant_integrand_and_combination_rules():
+    sec = SectorSpec([block(2, [], "1+0*x[1]")])
+    tr = []
+    val, sig, chi2, grid = integrate_vegas(sec, 1 << 11, SEED, nbins=16, iters=3, trace=tr)
+    assert float(tr[0]["I"][0, 0]) == 1.0 and float(tr[0]["var"][0, 0]) == 0.0       # uniform 2^-4 grid: W = 1 exactly
+    assert abs(float(val[0, 0]) - 1) <= 4 * float(sig[0, 0]) + 1e-15
+    val, sig, chi2, grid = integrate_vegas(sec, 1 << 11, SEED, nbins=10, iters=3)    # 1/10 inexact: clamp at 0
+    assert np.isfinite(float(sig[0, 0])) and float(sig[0, 0]) >= 0
+    assert abs(float(val[0, 0]) - 1) <= 4 * float(sig[0, 0]) + 1e-12
+    # hand numbers: I = (1, 3), var = (1, 4) -> value = (1 + 3/4)/(1 + 1/4) = 1.4, sigma^2 = 0.8, chi2 = 0.8
+    v, s, c = vegas_combine(np.array([[1.0], [3.0]], dtype=LD), np.array([[1.0], [4.0]], dtype=LD))
+    assert abs(float(v[0]) - 1.4) < 1e-15 and abs(float(s[0]) ** 2 - 0.8) < 1e-15 and abs(float(c[0]) - 0.8) < 1e-15
+    # all-zero variances: plain mean, sigma 0; partly zero: those take the smallest positive variance
+    v, s, c = vegas_combine(np.array([[1.0], [3.0]], dtype=LD), np.zeros((2, 1), dtype=LD))
+    assert float(v[0]) == 2 and float(s[0]) == 0
+    v, s, c = vegas_combine(np.array([[1.0], [3.0]], dtype=LD), np.array([[0.0], [4.0]], dtype=LD))
+    assert float(v[0]) == 2 and abs(float(s[0]) ** 2 - 2) < 1e-15
+
+
+def test_vegas_histogram_total_unbiasedness_and_adaptation():
+    # separable f = prod (1-a) x_i^-a, a = 0.4: exact integral 1; ideal edges (b/NB)^(1/(1-a))
+    a = 0.4
+    sec = SectorSpec([block(2, [], f"{(1 - a) ** 2!r}*p[x[1],{-a}]*p[x[2],{-a}]")])
+    tr = []
+    val, sig, chi2, grid = integrate_vegas(sec, 1 << 13, SEED, nbins=50, iters=8, trace=tr)
+    for rec in tr:
+        for d in range(2):
+            assert abs(float(np.sum(rec["hist"][d]) / rec["s2"][0, 0]) - 1) < 1e-15      # (iii): sum_b h = sum g^2
+            assert rec["grid"][d][0] == 0 and rec["grid"][d][-1] == 1 and np.all(np.diff(rec["grid"][d]) > 0)
+    assert abs(float(val[0, 0]) - 1) <= 4 * float(sig[0, 0])
+    sig_it = [math.sqrt(float(r["var"][0, 0])) for r in tr]
+    assert sig_it[-1] < 0.3 * sig_it[0]
+    ideal = (np.arange(51) / 50) ** (1 / (1 - a))
+    e0 = np.max(np.abs(tr[0]["grid"][0].astype(np.float64) - ideal))
+    e1 = np.max(np.abs(grid[0].astype(np.float64) - ideal))
+    assert e1 < 0.25 * e0
+    # (iv) unbiased on the adapted grid: a polynomial lands within 4 sigma of its closed form
+    sec2 = SectorSpec([block(2, [], "3*p[x[1],2]+x[2]")])
+    val, sig, chi2, _ = integrate_vegas(sec2, 1 << 12, SEED + 1, nbins=20, iters=5)
+    assert abs(float(val[0, 0]) - 1.5) <= 4 * float(sig[0, 0])
+
+
+def test_magnitude_companion_bounds_the_value():
+    prog = parse(block(2, ["1-x[1]+x[2]*0.5"], "l[f[1]]*(x[1]-x[2])/p[f[1],2.5]"))
+    rng = np.random.default_rng(10)
+    x = rng.uniform(0, 1, size=(200, 2))
+    v, m = evaluate_with_magnitude(prog, x)
+    assert np.all(m >= np.abs(v)) and np.all(v == evaluate(prog, x))
+    # sign-definite input without real powers or logs: M = |f|
+    prog = parse(block(2, ["1+x[1]+x[2]*0.5"], "x[1]*f[1]/p[f[1],3]+x[2]"))
+    v, m = evaluate_with_magnitude(prog, x)
+    assert np.max(np.abs(m / np.abs(v) - 1)) < 1e-17
+    # a cancelling argument makes M large relative to |f|
+    prog = parse(block(1, [], "(x[1]+1)-(x[1]+0.9999)"))
+    v, m = evaluate_with_magnitude(prog, x[:, :1])
+    assert np.all(m / np.abs(v) > 1e4)
