@@ -1,0 +1,190 @@
+/* fiesta_b200.h -- C ABI of the B200-native integration hot path of FIESTA 4 (arXiv:1511.03614).
+ *
+ * What the library does (citations: PAPER.md:<line> of the paper text, or DESIGN.md R<n> for a
+ * reading taken where the paper is silent):
+ *
+ *   fiesta_compile    turns the integrand expressions of each sector, one text per epsilon order in
+ *                     the integration worker's grammar, into a straight-line
+ *                     FP64 instruction program ("a sequence of quadripples (operator, first
+ *                     operand, second operand, result)") and uploads it to the GPU.
+ *   fiesta_integrate  evaluates every program at quasi-/pseudo-Monte-Carlo points generated on the
+ *                     device and reduces per sector and per order to (value, error)
+ *                     (PAPER.md:110, :118-124 for the evaluation; PAPER.md:316 for value +- error).
+ *
+ * Conventions
+ *   - every function returns 0 on success or a negative FIESTA_E_* code; no exception crosses
+ *     the ABI.  fiesta_last_error(ctx) gives a ctx-owned NUL-terminated message, valid until the
+ *     next call on that ctx.
+ *   - pointers named *_host are HOST memory, caller-allocated, borrowed for the call only.
+ *     pointers named *_dev are DEVICE memory on the ctx's device.
+ *   - calls are synchronous unless the name ends in _async: on return the stream has been
+ *     synchronised and host outputs are filled.
+ *   - there is no CPU fallback: without an sm_100 device fiesta_create fails with FIESTA_E_CUDA.
+ *   - all arithmetic is IEEE FP64 on the device.
+ */
+#ifndef FIESTA_B200_H
+#define FIESTA_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  FIESTA_OK = 0,
+  FIESTA_E_PARSE = -1,     /* text does not follow the grammar; message has sector/order/column   */
+  FIESTA_E_DIM = -2,       /* x[i] with i > dim, dim out of range, inconsistent nvars             */
+  FIESTA_E_NOTPOLY = -3,   /* deformation F is not a polynomial in x                              */
+  FIESTA_E_RULE = -4,      /* bad rule parameters (lattice size not 2^m, bins out of range, ...)  */
+  FIESTA_E_CUDA = -5,      /* CUDA runtime error or no suitable device                            */
+  FIESTA_E_NONFINITE = -6, /* some integrand value was NaN/Inf; results filled, n_nonfinite > 0   */
+  FIESTA_E_ARG = -7,       /* NULL pointer, bad index, size out of range                          */
+  FIESTA_E_TOOBIG = -8     /* a program exceeds the per-block shared-memory budget                */
+};
+
+#define FIESTA_MAX_DIM 12     /* integration variables per sector                                 */
+#define FIESTA_MAX_ORDERS 8   /* epsilon orders (outputs) per sector                              */
+#define FIESTA_MAX_BINS 128   /* Vegas bins per dimension                                         */
+
+typedef struct fiesta_ctx fiesta_ctx;         /* opaque; owns device scratch; bound to one device+stream */
+typedef struct fiesta_program fiesta_program; /* opaque; immutable after compile; free with _program_free */
+
+/* Create a context on CUDA device `cuda_device`.  `cuda_stream` is a cudaStream_t (may be 0 for
+ * the default stream); every launch and copy of this ctx goes to it. */
+int fiesta_create(fiesta_ctx **out, int cuda_device, void *cuda_stream);
+void fiesta_destroy(fiesta_ctx *ctx);
+const char *fiesta_last_error(const fiesta_ctx *ctx);
+
+/* One sector = K expression texts (one per epsilon order), each
+ *   "<nvars>;\n<nfunc>;\n<f1>;\n...\n<final>;\n|"
+ * with tokens: floats, x[i], f[i], + - * / ( ), p[expr,exponent], l[expr], P, G and the seven
+ * hard-coded PolyGamma[n,m].  The K texts of one sector may share f-lines; common
+ * subexpressions are evaluated once per point (R7).  An "evaluation" in the metric is
+ * still one (point, sector, order). */
+typedef struct {
+  int32_t sector_id;         /* caller's label; enters the random streams (R3)           */
+  int32_t n_orders;          /* K, 1..FIESTA_MAX_ORDERS                                            */
+  const char *const *expr;   /* K NUL-terminated texts                                             */
+  int32_t is_complex;        /* 0 real, 1 complex arithmetic                        */
+  int32_t deform_f_index;    /* >=1: f[deform_f_index] of text 0 is the polynomial F whose gradient
+                                drives the contour deformation (R11);
+                                0: no deformation.  Implies complex.                               */
+  double lambda;             /* deformation size; ignored if deform_f_index == 0                   */
+} fiesta_sector_desc;
+
+typedef struct {
+  int32_t n_ir_ops;          /* instructions of the main program                                   */
+  int32_t n_fp64_ops;        /* of which FP64 arithmetic (fma/mul/add/div/log/exp ...)             */
+  int32_t n_fma;             /* fused multiply-adds                                                */
+  int32_t n_log, n_exp, n_div;
+  int32_t n_reg_temps;       /* register temporaries used (of 8)                                   */
+  int32_t n_mem_slots;       /* shared-memory spill slots per point (compiler-directed; 0 is best) */
+  int32_t n_deform_ops;      /* instructions of the gradient/Hessian program (0 if none)           */
+  double flops;              /* FP64 flops per point counted as fma=2, mul/add=1, div=~15, log/exp~40 (nominal) */
+} fiesta_compile_info;
+
+/* Parse, optimise, register-allocate and upload.  `info` may be NULL, else [nsectors]. */
+int fiesta_compile(fiesta_ctx *ctx, const fiesta_sector_desc *sectors, int32_t nsectors, int32_t dim,
+                   fiesta_program **out, fiesta_compile_info *info);
+void fiesta_program_free(fiesta_program *prog);
+
+enum { FIESTA_RULE_LATTICE = 0, FIESTA_RULE_MC = 1, FIESTA_RULE_VEGAS = 2 };
+
+/* Sampling rule (R1-R4, R8; the paper names only "Vegas").
+ *   LATTICE: npoints = n_shifts * N_L, N_L = 2^m; rank-1 lattice with generating vector genvec
+ *            (or Korobov g_k = korobov_a^k mod N_L), n_shifts random shifts from Philox,
+ *            Korobov periodising transform of weight periodize_r (0..6).
+ *   MC:      npoints Philox points, x = u.
+ *   VEGAS:   vegas_iters iterations of npoints Philox points through a vegas_bins-bin grid per
+ *            dimension, refined between iterations with damping vegas_alpha. */
+typedef struct {
+  int32_t kind;
+  int32_t n_shifts;
+  uint64_t korobov_a;
+  const uint64_t *genvec;   /* optional HOST [dim]; NULL -> Korobov form */
+  int32_t periodize_r;
+  int32_t vegas_bins;
+  int32_t vegas_iters;
+  double vegas_alpha;
+} fiesta_rule;
+
+/* Per (sector, order).  Real sectors: im = im_err = 0.  chi2: Vegas only (else 0). */
+typedef struct {
+  double re, re_err, im, im_err, chi2;
+  uint64_t neval, n_nonfinite;
+} fiesta_result;
+
+/* Integrate sectors[0..nsectors) (indices into the program; NULL = 0..nsectors-1) and write
+ * out_host[nsectors][K] row-major.  All sectors of one call use the same rule and seed. */
+int fiesta_integrate(fiesta_ctx *ctx, const fiesta_program *prog, const int32_t *sectors, int32_t nsectors,
+                     int32_t dim, uint64_t npoints, const fiesta_rule *rule, uint64_t seed,
+                     fiesta_result *out_host);
+
+/* Same work, but nothing is copied back and the stream is not synchronised; results stay in a
+ * ctx-owned device buffer that fiesta_fetch_results copies out.  For device-side timing. */
+int fiesta_integrate_async(fiesta_ctx *ctx, const fiesta_program *prog, const int32_t *sectors, int32_t nsectors,
+                           int32_t dim, uint64_t npoints, const fiesta_rule *rule, uint64_t seed);
+int fiesta_fetch_results(fiesta_ctx *ctx, int32_t nsectors, int32_t K, fiesta_result *out_host);
+
+/* Device time (ms, CUDA events on the ctx stream) that the evaluation kernel(s) of the last
+ * fiesta_integrate[_async] took, and how many kernels the call launched.  Synchronises. */
+int fiesta_last_timing(fiesta_ctx *ctx, double *eval_kernel_ms, int32_t *n_launches);
+
+/* ---- parity hooks: the same device code paths, exposed piecewise -------------------------- */
+
+/* Integrand values at caller-given points (PAPER.md:414 `justEvaluate`; PAPER.md:531 `Debug`).
+ * x_host[npts][dim]; out_host[npts][K][2] = (re, im) of o_k(x) -- for deformed sectors
+ * o_k(z(x)) * det J(x) -- WITHOUT the rule's weight. */
+int fiesta_eval_points(fiesta_ctx *ctx, const fiesta_program *prog, int32_t sector, const double *x_host,
+                       uint64_t npts, double *out_host);
+
+/* The 64-bit integers t[j][k] (R2/R3) behind points j = first..first+count-1 of shift
+ * (lattice) or iteration (MC/Vegas) `shift_or_iter` of the sector labelled sector_id.
+ * n_lattice is used by the lattice rule only.  t_host[count][dim]. */
+int fiesta_generate_points(fiesta_ctx *ctx, const fiesta_rule *rule, uint64_t seed, int32_t sector_id,
+                           int32_t shift_or_iter, uint64_t n_lattice, uint64_t first, uint64_t count,
+                           int32_t dim, uint64_t *t_host);
+
+/* The unit-cube point and weight the rule makes from those integers (lattice: after the
+ * periodising transform; MC: x = u, w = 1).  x_host[count][dim], xbar_host[count][dim] (= 1 - x,
+ * computed without cancellation), w_host[count]. */
+int fiesta_transform_points(fiesta_ctx *ctx, const fiesta_rule *rule, const uint64_t *t_host, uint64_t count,
+                            int32_t dim, double *x_host, double *xbar_host, double *w_host);
+
+/* Lattice / MC: per-shift sums S1 = sum_j g, S2 = sum_j g^2, g = W * o_k component, before the
+ * estimator.  sums_host[nsectors][R][K][C][2], C = 1 (real) or 2 (complex: Re, Im). */
+int fiesta_partial_sums(fiesta_ctx *ctx, const fiesta_program *prog, const int32_t *sectors, int32_t nsectors,
+                        int32_t dim, uint64_t npoints, const fiesta_rule *rule, uint64_t seed,
+                        double *sums_host);
+
+/* One Vegas iteration of one sector on a caller-given grid (R8):
+ * grid_host[dim][NB+1] in; sums_host[K][C][2] (S1, S2) and hist_host[dim][NB] out. */
+int fiesta_vegas_iteration(fiesta_ctx *ctx, const fiesta_program *prog, int32_t sector, int32_t dim,
+                           uint64_t npoints, const fiesta_rule *rule, uint64_t seed, int32_t iteration,
+                           const double *grid_host, double *sums_host, double *hist_host);
+
+/* The grid refinement step alone: ngrids independent (grid[NB+1], hist[NB]) pairs. */
+int fiesta_vegas_refine(fiesta_ctx *ctx, int32_t ngrids, int32_t nbins, double alpha, const double *grid_host,
+                        const double *hist_host, double *grid_out_host);
+
+/* Grid and last histogram of sector index `sector` after the last VEGAS fiesta_integrate.
+ * grid_host[dim][NB+1], hist_host[dim][NB] (either may be NULL). */
+int fiesta_vegas_grid(fiesta_ctx *ctx, int32_t sector, int32_t dim, int32_t nbins, double *grid_host,
+                      double *hist_host);
+
+/* Sum over sectors with errors combined in mean square.  Host arithmetic on
+ * nsectors*K numbers; total_host[K]. */
+int fiesta_combine(const fiesta_result *per_sector_host, int32_t nsectors, int32_t K, fiesta_result *total_host);
+
+/* Disassembly of a compiled sector (main program, then the deformation program) into buf. */
+int fiesta_program_dump(const fiesta_program *prog, int32_t sector, char *buf_host, uint64_t buflen);
+
+/* FP64 pipe micro-benchmark: independent DFMA chains on every SM for about `ms_target`
+ * milliseconds; writes achieved TFLOP/s (2 flops per DFMA).  The roofline denominator. */
+int fiesta_fp64_peak(fiesta_ctx *ctx, double ms_target, double *tflops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FIESTA_B200_H */
