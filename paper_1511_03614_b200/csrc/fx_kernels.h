@@ -1,0 +1,104 @@
+// fx_kernels.h -- launch interface between the C ABI (host) and the sm_100a kernels.
+#ifndef FX_KERNELS_H
+#define FX_KERNELS_H
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "fx_isa.h"
+
+#define FX_THREADS 128   // threads per block of the evaluation kernels
+#define FX_P_REAL 4      // points per thread, real programs
+#define FX_P_CPLX 2      // points per thread, complex programs
+#define FX_ACC_SLOTS 32  // per-(sector,shift,chunk) partial record: [K<=8][C<=2][S1,S2]
+
+struct fx_sector_dev {       // one compiled sector in the device arena
+  uint32_t main_off;         // instruction index of the main program in the arena
+  uint32_t main_len;         // instructions incl. FX_END and one pad
+  uint32_t deform_off;
+  uint32_t deform_len;       // 0: no deformation
+  int32_t K;
+  int32_t is_complex;
+  int32_t sector_id;
+  int32_t n_mem_main;        // spill slots (scalars of the program's type)
+  int32_t n_mem_deform;      // spill slots (doubles) incl. the gradient/Hessian outputs
+  int32_t pad;
+  double lambda;
+};
+
+struct fx_transform_host {
+  int r;
+  double cw;
+  double coef[7];
+};
+
+struct fx_integrate_params {
+  const fx_ins *arena;
+  const fx_sector_dev *sectors;
+  const int32_t *sel;        // device: selected sector indices [nsel]
+  int32_t nsel;
+  int32_t dim;
+  int32_t rule;              // FIESTA_RULE_*
+  int32_t n_shifts;          // R (lattice) or 1
+  uint64_t n_per_shift;      // N_L (lattice) or points per iteration (MC / Vegas)
+  int32_t log2_n;            // m (lattice)
+  uint64_t chunk;            // points per block
+  int32_t nchunks;
+  int32_t iteration;         // Vegas iteration / MC stream index
+  uint64_t genvec[FX_NXMAX];
+  fx_transform_host tf;
+  uint64_t seed;
+  int32_t nbins;
+  const double *grid;        // Vegas: [nsel][dim][nbins+1]
+  double *hist;              // Vegas: [nsel][dim][nbins]
+  double *partials;          // [nsel][R][nchunks][FX_ACC_SLOTS]
+  unsigned long long *nonfinite;  // [nsel]
+  int32_t mem_doubles;       // shared-memory spill doubles per block (all threads)
+  int32_t prog_ins_max;      // instructions reserved in shared memory (main + deform)
+};
+
+struct fx_eval_params {
+  const fx_ins *arena;
+  const fx_sector_dev *sectors;
+  int32_t sector;
+  int32_t dim;
+  uint64_t npts;
+  const double *x;           // device [npts][dim]
+  double *out;               // device [npts][K][2]
+  int32_t mem_doubles;
+  int32_t prog_ins_max;
+};
+
+size_t fx_integrate_smem_bytes(const fx_integrate_params &p);
+
+// S[nsel][R][FX_ACC_SLOTS] = sum over chunks of the partials, fixed order
+cudaError_t fx_launch_reduce_chunks(const double *partials, double *sums, int nsel, int R, int nchunks, cudaStream_t st);
+
+struct fx_result_dev {
+  double re, re_err, im, im_err, chi2;
+  unsigned long long neval, n_nonfinite;
+};
+// lattice / MC estimator (R5) -> results[nsel][K]
+cudaError_t fx_launch_estimate(const double *sums, const fx_sector_dev *sectors, const int32_t *sel, int nsel, int R,
+                               uint64_t n_per_shift, const unsigned long long *nonfinite, fx_result_dev *results,
+                               int Kstride, cudaStream_t st);
+// Vegas: per-iteration (I, var) from the sums of one iteration -> iter_stats[it][nsel][FX_ACC_SLOTS]
+cudaError_t fx_launch_vegas_iter_stats(const double *sums, double *iter_stats, int it, int nsel, uint64_t npoints,
+                                       cudaStream_t st);
+cudaError_t fx_launch_vegas_combine(const double *iter_stats, int iters, const fx_sector_dev *sectors,
+                                    const int32_t *sel, int nsel, uint64_t npoints,
+                                    const unsigned long long *nonfinite, fx_result_dev *results, int Kstride,
+                                    cudaStream_t st);
+// refine ngrids independent (grid[NB+1], hist[NB]) pairs (R8 i-iv); in place allowed
+cudaError_t fx_launch_vegas_refine(const double *grid_in, const double *hist, double *grid_out, int ngrids, int nbins,
+                                   double alpha, cudaStream_t st);
+cudaError_t fx_launch_vegas_init_grid(double *grid, int ngrids, int nbins, cudaStream_t st);
+
+cudaError_t fx_launch_generate_points(int rule, uint64_t seed, int sector_id, int shift_or_iter, uint64_t n_lattice,
+                                      int log2_n, const uint64_t *genvec_host, uint64_t first, uint64_t count, int dim,
+                                      uint64_t *t_dev, cudaStream_t st);
+cudaError_t fx_launch_transform_points(int rule, const fx_transform_host &tf, const uint64_t *t_dev, uint64_t count,
+                                       int dim, double *x_dev, double *xbar_dev, double *w_dev, cudaStream_t st);
+cudaError_t fx_launch_fp64_peak(double *sink_dev, int iters, int blocks, cudaStream_t st);
+
+#endif

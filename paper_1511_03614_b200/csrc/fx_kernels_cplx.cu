@@ -1,0 +1,261 @@
+// fx_kernels_cplx.cu -- evaluation kernels for complex sectors ("-complex"), with
+// the contour deformation of the physical region (formula DESIGN.md R11):
+//     g_k  = dF/dx_k (x)                                  real program (FX_STM outputs)
+//     z_k  = x_k - i*lambda*x_k*(1-x_k)*g_k
+//     J_kl = delta_kl (1 - i*lambda*(1-2x_k) g_k) - i*lambda*x_k(1-x_k) d2F/dx_k dx_l
+//     o_k(z) * det J                                      complex program, LU with partial pivoting
+// Compiled once per dimension N (-DFX_N=1..8) so the N x N elimination is fully unrolled on
+// registers.  SURVEY 8(a) steps A4, A5 (complex), A6, A7.
+#include "fx_device_common.cuh"
+
+#ifndef FX_N
+#error "compile with -DFX_N=<dimension 1..8>"
+#endif
+
+namespace {
+
+constexpr int N = FX_N;
+constexpr int P = FX_P_CPLX;
+constexpr int NGH = N + N * (N + 1) / 2;  // gradient + upper Hessian slots written by the deform program
+
+struct NoSink {
+  __device__ __forceinline__ void operator()(int, double (&)[P]) {}
+};
+
+__device__ __forceinline__ int hess_slot(int k, int l) {  // k <= l, row-major upper triangle after the gradient
+  return N + k * N - k * (k - 1) / 2 + (l - k);
+}
+
+// det of J (complex N x N, registers) by LU with partial pivoting on |.|^2 (R12)
+__device__ __forceinline__ cplx det_lu(cplx (&J)[N][N]) {
+  cplx det{1.0, 0.0};
+#pragma unroll
+  for (int c = 0; c < N; ++c) {
+#pragma unroll
+    for (int r = c + 1; r < N; ++r) {
+      const double mc = fma(J[c][c].re, J[c][c].re, J[c][c].im * J[c][c].im);
+      const double mr = fma(J[r][c].re, J[r][c].re, J[r][c].im * J[r][c].im);
+      if (mr > mc) {
+#pragma unroll
+        for (int l = c; l < N; ++l) {
+          const cplx t = J[c][l];
+          J[c][l] = J[r][l];
+          J[r][l] = t;
+        }
+        det = t_neg(det);
+      }
+    }
+    const cplx piv = J[c][c];
+    det = t_mul(det, piv);
+    const cplx inv = t_rdivc(1.0, piv);
+#pragma unroll
+    for (int r = c + 1; r < N; ++r) {
+      const cplx m = t_mul(J[r][c], inv);
+      const cplx mn = t_neg(m);
+#pragma unroll
+      for (int l = c + 1; l < N; ++l) J[r][l] = t_fma(mn, J[c][l], J[r][l]);
+    }
+  }
+  return det;
+}
+
+// x (real, registers) -> X = z(x) (complex) and det J per point.  sh_deform == nullptr: z = x, det = 1.
+__device__ __forceinline__ void fx_deform_points(const fx_ins *sh_deform, double lambda, double (&x)[N][P],
+                                                 double (&xbar)[N][P], const fx_mem<double> M, cplx (&X)[N][P],
+                                                 cplx (&det)[P]) {
+  if (sh_deform == nullptr) {
+#pragma unroll
+    for (int k = 0; k < N; ++k) FX_PLOOP { X[k][p] = cplx{x[k][p], 0.0}; }
+    FX_PLOOP { det[p] = cplx{1.0, 0.0}; }
+    return;
+  }
+  NoSink ns;
+  fx_run<double, N, P>(sh_deform, x, M, ns);  // M[0..NGH) = gradient, upper Hessian
+#pragma unroll
+  for (int k = 0; k < N; ++k) FX_PLOOP {
+      M.st(NGH + k, p, P, x[k][p]);
+      M.st(NGH + N + k, p, P, xbar[k][p]);
+    }
+#pragma unroll 1
+  for (int p = 0; p < P; ++p) {  // one matrix at a time: 2*N*N doubles in registers
+    cplx J[N][N];
+    double zi[N];
+#pragma unroll
+    for (int k = 0; k < N; ++k) {
+      const double xk = M.ld(NGH + k, p, P), xb = M.ld(NGH + N + k, p, P), gk = M.ld(k, p, P);
+      const double ls = lambda * (xk * xb);
+      zi[k] = -(ls * gk);
+#pragma unroll
+      for (int l = 0; l < N; ++l) {
+        const double h = M.ld(k <= l ? hess_slot(k, l) : hess_slot(l, k), p, P);
+        J[k][l] = cplx{0.0, -(ls * h)};
+      }
+      J[k][k].re = 1.0;
+      J[k][k].im -= lambda * (xb - xk) * gk;  // 1 - 2x = xbar - x
+    }
+    const cplx d = det_lu(J);
+#pragma unroll
+    for (int k = 0; k < N; ++k) M.st(k, p, P, zi[k]);
+    M.st(NGH, p, P, d.re);
+    M.st(NGH + (N > 1 ? 1 : N), p, P, d.im);
+  }
+#pragma unroll
+  for (int k = 0; k < N; ++k) FX_PLOOP { X[k][p] = cplx{x[k][p], M.ld(k, p, P)}; }
+  FX_PLOOP { det[p] = cplx{M.ld(NGH, p, P), M.ld(NGH + (N > 1 ? 1 : N), p, P)}; }
+}
+
+struct IntegrateSinkCplx {
+  double *acc;
+  const cplx (&Wd)[P];  // weight * det J
+  unsigned valid;
+  unsigned nonfinite;
+  double (&h2)[P];
+  __device__ __forceinline__ void operator()(int k, cplx (&A)[P]) {
+    double s1r = acc[(4 * k) * FX_THREADS], s2r = acc[(4 * k + 1) * FX_THREADS];
+    double s1i = acc[(4 * k + 2) * FX_THREADS], s2i = acc[(4 * k + 3) * FX_THREADS];
+    FX_PLOOP {
+      cplx g = t_mul(Wd[p], A[p]);
+      if (!((valid >> p) & 1u)) g = cplx{0.0, 0.0};
+      nonfinite += (isfinite(g.re) && isfinite(g.im)) ? 0u : 1u;
+      s1r += g.re;
+      s2r = fma(g.re, g.re, s2r);
+      s1i += g.im;
+      s2i = fma(g.im, g.im, s2i);
+      h2[p] = fma(g.re, g.re, fma(g.im, g.im, h2[p]));
+    }
+    acc[(4 * k) * FX_THREADS] = s1r;
+    acc[(4 * k + 1) * FX_THREADS] = s2r;
+    acc[(4 * k + 2) * FX_THREADS] = s1i;
+    acc[(4 * k + 3) * FX_THREADS] = s2i;
+  }
+};
+
+__global__ void __launch_bounds__(FX_THREADS) fx_integrate_cplx(const __grid_constant__ fx_integrate_params prm) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  const int b = blockIdx.x;
+  const int chunk = b % prm.nchunks;
+  const int r = (b / prm.nchunks) % prm.n_shifts;
+  const int sel_idx = b / (prm.nchunks * prm.n_shifts);
+  const fx_sector_dev sec = prm.sectors[prm.sel[sel_idx]];
+  if (!sec.is_complex) return;
+  const bool vegas = prm.rule == FIESTA_RULE_VEGAS;
+  const fx_smem_layout L = fx_layout(prm.prog_ins_max, prm.mem_doubles, N, prm.nbins, vegas);
+  fx_ins *sh_prog = reinterpret_cast<fx_ins *>(smem + L.prog);
+  fx_ins *sh_deform = sec.deform_len ? sh_prog + sec.main_len : nullptr;
+  double *sh_mem = reinterpret_cast<double *>(smem + L.mem);
+  double *sh_acc = reinterpret_cast<double *>(smem + L.acc);
+  uint64_t *sh_delta = reinterpret_cast<uint64_t *>(smem + L.delta);
+  double *sh_grid = reinterpret_cast<double *>(smem + L.grid);
+  double *sh_hist = reinterpret_cast<double *>(smem + L.hist);
+  double *sh_wsum = reinterpret_cast<double *>(smem + L.wsum);
+
+  fx_copy_program(sh_prog, prm.arena + sec.main_off, sec.main_len);
+  if (sec.deform_len) fx_copy_program(sh_deform, prm.arena + sec.deform_off, sec.deform_len);
+  fx_block_setup(prm, N, (uint32_t)sec.sector_id, r, sel_idx, sh_delta, sh_grid, sh_hist);
+  const int nslots = 4 * sec.K;
+  for (int s = 0; s < nslots; ++s) sh_acc[s * FX_THREADS + threadIdx.x] = 0.0;
+  __syncthreads();
+
+  const uint64_t c0 = (uint64_t)chunk * prm.chunk;
+  const uint64_t c1 = min(c0 + prm.chunk, prm.n_per_shift);
+  const fx_mem<double> Mr{sh_mem + threadIdx.x, FX_THREADS};
+  const fx_mem<cplx> Mc{sh_mem + threadIdx.x, FX_THREADS};
+  unsigned nonfinite = 0;
+  for (uint64_t base = c0 + (uint64_t)threadIdx.x * P; base < c1; base += (uint64_t)FX_THREADS * P) {
+    double x[N][P], xbar[N][P], W[P], h2[P];
+    uint32_t bins[(N + 3) / 4][P];
+    unsigned valid;
+    fx_make_points<N, P>(prm, N, (uint32_t)sec.sector_id, sh_delta, sh_grid, base, c1, x, xbar, W, valid, bins);
+    cplx X[N][P], Wd[P];
+    fx_deform_points(sh_deform, sec.lambda, x, xbar, Mr, X, Wd);
+    FX_PLOOP {
+      Wd[p] = t_mulc(Wd[p], W[p]);
+      h2[p] = 0.0;
+    }
+    IntegrateSinkCplx sink{sh_acc + threadIdx.x, Wd, valid, 0u, h2};
+    fx_run<cplx, N, P>(sh_prog, X, Mc, sink);
+    nonfinite += sink.nonfinite;
+    if (vegas) {
+      FX_PLOOP {
+        if ((valid >> p) & 1u) {
+#pragma unroll
+          for (int k = 0; k < N; ++k)
+            atomicAdd(sh_hist + k * prm.nbins + ((bins[k / 4][p] >> (8 * (k % 4))) & 0xffu), h2[p]);
+        }
+      }
+    }
+  }
+  __syncthreads();
+  double *out = prm.partials + (((size_t)sel_idx * prm.n_shifts + r) * prm.nchunks + chunk) * FX_ACC_SLOTS;
+  fx_block_reduce(sh_acc, sh_wsum, nslots, out);
+  fx_block_finish(prm, N, sel_idx, nonfinite, sh_hist);
+}
+
+struct EvalSinkCplx {
+  double *out;
+  int K;
+  unsigned valid;
+  const cplx (&det)[P];
+  __device__ __forceinline__ void operator()(int k, cplx (&A)[P]) {
+    FX_PLOOP {
+      if ((valid >> p) & 1u) {
+        const cplx v = t_mul(det[p], A[p]);
+        out[((size_t)p * K + k) * 2] = v.re;
+        out[((size_t)p * K + k) * 2 + 1] = v.im;
+      }
+    }
+  }
+};
+
+__global__ void __launch_bounds__(FX_THREADS) fx_eval_cplx(const __grid_constant__ fx_eval_params prm) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  const fx_sector_dev sec = prm.sectors[prm.sector];
+  fx_ins *sh_prog = reinterpret_cast<fx_ins *>(smem);
+  fx_ins *sh_deform = sec.deform_len ? sh_prog + sec.main_len : nullptr;
+  double *sh_mem = reinterpret_cast<double *>(smem + (size_t)prm.prog_ins_max * 16);
+  fx_copy_program(sh_prog, prm.arena + sec.main_off, sec.main_len);
+  if (sec.deform_len) fx_copy_program(sh_deform, prm.arena + sec.deform_off, sec.deform_len);
+  __syncthreads();
+  const uint64_t first = ((uint64_t)blockIdx.x * FX_THREADS + threadIdx.x) * P;
+  if (first >= prm.npts) return;
+  double x[N][P], xbar[N][P];
+  unsigned valid = 0;
+  FX_PLOOP {
+    const bool ok = first + p < prm.npts;
+    if (ok) valid |= 1u << p;
+#pragma unroll
+    for (int k = 0; k < N; ++k) {
+      x[k][p] = ok ? prm.x[(first + p) * N + k] : 0.5;
+      xbar[k][p] = 1.0 - x[k][p];
+    }
+  }
+  const fx_mem<double> Mr{sh_mem + threadIdx.x, FX_THREADS};
+  const fx_mem<cplx> Mc{sh_mem + threadIdx.x, FX_THREADS};
+  cplx X[N][P], det[P];
+  fx_deform_points(sh_deform, sec.lambda, x, xbar, Mr, X, det);
+  EvalSinkCplx sink{prm.out + first * sec.K * 2, sec.K, valid, det};
+  fx_run<cplx, N, P>(sh_prog, X, Mc, sink);
+}
+
+}  // namespace
+
+#define FX_CAT2(a, b) a##b
+#define FX_CAT(a, b) FX_CAT2(a, b)
+
+cudaError_t FX_CAT(fx_launch_integrate_cplx_n, FX_N)(const fx_integrate_params &prm, size_t smem, cudaStream_t st) {
+  cudaError_t e = cudaFuncSetAttribute(fx_integrate_cplx, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  const unsigned grid = (unsigned)((size_t)prm.nsel * prm.n_shifts * prm.nchunks);
+  fx_integrate_cplx<<<grid, FX_THREADS, smem, st>>>(prm);
+  return cudaGetLastError();
+}
+
+cudaError_t FX_CAT(fx_launch_eval_cplx_n, FX_N)(const fx_eval_params &prm, size_t smem, cudaStream_t st) {
+  cudaError_t e = cudaFuncSetAttribute(fx_eval_cplx, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  const uint64_t per_block = (uint64_t)FX_THREADS * P;
+  const unsigned grid = (unsigned)((prm.npts + per_block - 1) / per_block);
+  if (grid == 0) return cudaSuccess;
+  fx_eval_cplx<<<grid, FX_THREADS, smem, st>>>(prm);
+  return cudaGetLastError();
+}

@@ -1,0 +1,169 @@
+// fx_kernels_real.cu -- evaluation kernels for real (Euclidean) sectors: lattice / MC / Vegas
+// points made on the device, program walk, accumulation of sum g and sum g^2 per order
+// (SURVEY 8(a) A1-A3, A5-A7, A8 histogram part).  Replaces the reference's CUDA kernel of
+// PAPER.md:118-126 (thread per point, temporaries in GPU memory, points uploaded per batch).
+#include "fx_device_common.cuh"
+
+namespace {
+
+template <int P>
+struct IntegrateSinkReal {
+  double *acc;  // &acc[0][tid], slot stride FX_THREADS
+  const double (&W)[P];
+  unsigned valid;
+  unsigned nonfinite;
+  double (&h2)[P];
+  __device__ __forceinline__ void operator()(int k, double (&A)[P]) {
+    double s1 = acc[(2 * k) * FX_THREADS], s2 = acc[(2 * k + 1) * FX_THREADS];
+    FX_PLOOP {
+      double g = W[p] * A[p];
+      if (!((valid >> p) & 1u)) g = 0.0;
+      nonfinite += isfinite(g) ? 0u : 1u;
+      s1 += g;
+      s2 = fma(g, g, s2);
+      h2[p] = fma(g, g, h2[p]);
+    }
+    acc[(2 * k) * FX_THREADS] = s1;
+    acc[(2 * k + 1) * FX_THREADS] = s2;
+  }
+};
+
+template <int NX>
+__global__ void __launch_bounds__(FX_THREADS) fx_integrate_real(const __grid_constant__ fx_integrate_params prm) {
+  constexpr int P = FX_P_REAL;
+  extern __shared__ __align__(16) unsigned char smem[];
+  const int b = blockIdx.x;
+  const int chunk = b % prm.nchunks;
+  const int r = (b / prm.nchunks) % prm.n_shifts;
+  const int sel_idx = b / (prm.nchunks * prm.n_shifts);
+  const fx_sector_dev sec = prm.sectors[prm.sel[sel_idx]];
+  if (sec.is_complex) return;
+  const int dim = prm.dim;
+  const bool vegas = prm.rule == FIESTA_RULE_VEGAS;
+  const fx_smem_layout L = fx_layout(prm.prog_ins_max, prm.mem_doubles, dim, prm.nbins, vegas);
+  fx_ins *sh_prog = reinterpret_cast<fx_ins *>(smem + L.prog);
+  double *sh_mem = reinterpret_cast<double *>(smem + L.mem);
+  double *sh_acc = reinterpret_cast<double *>(smem + L.acc);
+  uint64_t *sh_delta = reinterpret_cast<uint64_t *>(smem + L.delta);
+  double *sh_grid = reinterpret_cast<double *>(smem + L.grid);
+  double *sh_hist = reinterpret_cast<double *>(smem + L.hist);
+  double *sh_wsum = reinterpret_cast<double *>(smem + L.wsum);
+
+  fx_copy_program(sh_prog, prm.arena + sec.main_off, sec.main_len);
+  fx_block_setup(prm, dim, (uint32_t)sec.sector_id, r, sel_idx, sh_delta, sh_grid, sh_hist);
+  const int nslots = 2 * sec.K;
+  for (int s = 0; s < nslots; ++s) sh_acc[s * FX_THREADS + threadIdx.x] = 0.0;
+  __syncthreads();
+
+  const uint64_t c0 = (uint64_t)chunk * prm.chunk;
+  const uint64_t c1 = min(c0 + prm.chunk, prm.n_per_shift);
+  const fx_mem<double> M{sh_mem + threadIdx.x, FX_THREADS};
+  unsigned nonfinite = 0;
+  for (uint64_t base = c0 + (uint64_t)threadIdx.x * P; base < c1; base += (uint64_t)FX_THREADS * P) {
+    double x[NX][P], xbar[NX][P], W[P], h2[P];
+    uint32_t bins[(NX + 3) / 4][P];
+    unsigned valid;
+    fx_make_points<NX, P>(prm, dim, (uint32_t)sec.sector_id, sh_delta, sh_grid, base, c1, x, xbar, W, valid, bins);
+    FX_PLOOP { h2[p] = 0.0; }
+    IntegrateSinkReal<P> sink{sh_acc + threadIdx.x, W, valid, 0u, h2};
+    fx_run<double, NX, P>(sh_prog, x, M, sink);
+    nonfinite += sink.nonfinite;
+    if (vegas) {
+      FX_PLOOP {
+        if ((valid >> p) & 1u) {
+#pragma unroll
+          for (int k = 0; k < NX; ++k)
+            if (k < dim) atomicAdd(sh_hist + k * prm.nbins + ((bins[k / 4][p] >> (8 * (k % 4))) & 0xffu), h2[p]);
+        }
+      }
+    }
+  }
+  __syncthreads();
+  double *out = prm.partials + (((size_t)sel_idx * prm.n_shifts + r) * prm.nchunks + chunk) * FX_ACC_SLOTS;
+  fx_block_reduce(sh_acc, sh_wsum, nslots, out);
+  fx_block_finish(prm, dim, sel_idx, nonfinite, sh_hist);
+}
+
+template <int P>
+struct EvalSinkReal {
+  double *out;  // &out[first point of this thread][0][0]
+  int K;
+  unsigned valid;
+  __device__ __forceinline__ void operator()(int k, double (&A)[P]) {
+    FX_PLOOP {
+      if ((valid >> p) & 1u) {
+        out[((size_t)p * K + k) * 2] = A[p];
+        out[((size_t)p * K + k) * 2 + 1] = 0.0;
+      }
+    }
+  }
+};
+
+template <int NX>
+__global__ void __launch_bounds__(FX_THREADS) fx_eval_real(const __grid_constant__ fx_eval_params prm) {
+  constexpr int P = FX_P_REAL;
+  extern __shared__ __align__(16) unsigned char smem[];
+  const fx_sector_dev sec = prm.sectors[prm.sector];
+  fx_ins *sh_prog = reinterpret_cast<fx_ins *>(smem);
+  double *sh_mem = reinterpret_cast<double *>(smem + (size_t)prm.prog_ins_max * 16);
+  fx_copy_program(sh_prog, prm.arena + sec.main_off, sec.main_len);
+  __syncthreads();
+  const uint64_t first = ((uint64_t)blockIdx.x * FX_THREADS + threadIdx.x) * P;
+  if (first >= prm.npts) return;
+  double x[NX][P];
+  unsigned valid = 0;
+  FX_PLOOP {
+    const bool ok = first + p < prm.npts;
+    if (ok) valid |= 1u << p;
+#pragma unroll
+    for (int k = 0; k < NX; ++k) x[k][p] = (ok && k < prm.dim) ? prm.x[(first + p) * prm.dim + k] : 0.5;
+  }
+  const fx_mem<double> M{sh_mem + threadIdx.x, FX_THREADS};
+  EvalSinkReal<P> sink{prm.out + first * sec.K * 2, sec.K, valid};
+  fx_run<double, NX, P>(sh_prog, x, M, sink);
+}
+
+template <typename K>
+cudaError_t set_smem(K kernel, size_t bytes) {
+  return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+}  // namespace
+
+size_t fx_integrate_smem_bytes(const fx_integrate_params &prm) {
+  return fx_layout(prm.prog_ins_max, prm.mem_doubles, prm.dim, prm.nbins, prm.rule == FIESTA_RULE_VEGAS).total;
+}
+
+cudaError_t fx_launch_integrate_real(const fx_integrate_params &prm, cudaStream_t st) {
+  const size_t smem = fx_integrate_smem_bytes(prm);
+  const unsigned grid = (unsigned)((size_t)prm.nsel * prm.n_shifts * prm.nchunks);
+  cudaError_t e;
+#define FX_LAUNCH(NX)                                                             \
+  {                                                                               \
+    if ((e = set_smem(fx_integrate_real<NX>, smem)) != cudaSuccess) return e;     \
+    fx_integrate_real<NX><<<grid, FX_THREADS, smem, st>>>(prm);                     \
+  }
+  if (prm.dim <= 4) FX_LAUNCH(4)
+  else if (prm.dim <= 8) FX_LAUNCH(8)
+  else FX_LAUNCH(12)
+#undef FX_LAUNCH
+  return cudaGetLastError();
+}
+
+cudaError_t fx_launch_eval_real(const fx_eval_params &prm, cudaStream_t st) {
+  const size_t smem = (size_t)prm.prog_ins_max * 16 + (size_t)prm.mem_doubles * 8;
+  const uint64_t per_block = (uint64_t)FX_THREADS * FX_P_REAL;
+  const unsigned grid = (unsigned)((prm.npts + per_block - 1) / per_block);
+  if (grid == 0) return cudaSuccess;
+  cudaError_t e;
+#define FX_LAUNCH(NX)                                                        \
+  {                                                                          \
+    if ((e = set_smem(fx_eval_real<NX>, smem)) != cudaSuccess) return e;     \
+    fx_eval_real<NX><<<grid, FX_THREADS, smem, st>>>(prm);                     \
+  }
+  if (prm.dim <= 4) FX_LAUNCH(4)
+  else if (prm.dim <= 8) FX_LAUNCH(8)
+  else FX_LAUNCH(12)
+#undef FX_LAUNCH
+  return cudaGetLastError();
+}
