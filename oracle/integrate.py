@@ -88,16 +88,19 @@ def lattice_points(sec: SectorSpec, n_lattice, genvec, r_periodize, seed, shift_
     return x, xbar, np.prod(w, axis=1)
 
 
-def lattice_partial_sums(sec: SectorSpec, n_lattice, n_shifts, genvec, r_periodize, seed, chunk=1 << 14, rdtype=LD):
+def lattice_partial_sums(sec: SectorSpec, n_lattice, n_shifts, genvec, r_periodize, seed, chunk=1 << 14, rdtype=LD,
+                         shifts=None):
     """S1[r,k,c] = sum_j g, S2[r,k,c] = sum_j g^2, SA[r,k,c] = sum_j |g|, g = W*o_k component c.
 
     Shapes [R, K, C], C = 1 (real) or 2 (Re, Im).  Sums run in index order over j (O6).
+    `shifts`: optional subset of shift indices to compute (the other rows stay 0); used to
+    sample single shifts of a full-size run.
     """
     ncomp = 2 if (sec.is_complex or sec.deform_f_index > 0) else 1
     s1 = np.zeros((n_shifts, sec.K, ncomp), dtype=rdtype)
     s2 = np.zeros_like(s1)
     sa = np.zeros_like(s1)
-    for r in range(n_shifts):
+    for r in (range(n_shifts) if shifts is None else shifts):
         parts = [[[[], [], []] for _ in range(ncomp)] for _ in range(sec.K)]
         for first in range(0, n_lattice, chunk):
             cnt = min(chunk, n_lattice - first)

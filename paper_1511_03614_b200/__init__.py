@@ -9,3 +9,5 @@ from .binding import (  # noqa: F401
     Context, Program, Rule, FiestaError, LIB_PATH, load_library, exported_symbols,
     RULE_LATTICE, RULE_MC, RULE_VEGAS, RESULT_DTYPE, INFO_DTYPE,
 )
+
+load = load_library

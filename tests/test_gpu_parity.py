@@ -1,0 +1,514 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element
+on the same seeded inputs.  Run with `-m gpu` on the B200 box.
+
+Bars (BASELINE.json north_star; readings R14/R15 in DESIGN.md):
+  integers t (points)         bit-exact
+  per-point values            |diff| <= 1e-12 * M(x)
+  per-shift sums              |diff| <= 1e-10 |S| + 1e-13 sum|g|
+  closed forms                within 4 sigma of the reported error
+"""
+import numpy as np
+import pytest
+
+from workloads import make_workload, SectorText
+from oracle import integrate as OI
+from oracle import points as OP
+from oracle.integrate import SectorSpec
+
+from helpers import (LD, TOL_POINT, check_points, check_sums, genvec_of, oracle_values_and_magnitude, spec)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def fb(lib):
+    return lib
+
+
+@pytest.fixture(scope="module")
+def ctx(fb):
+    c = fb.Context(0)
+    yield c
+    c.close()
+
+
+def block(nvars, flines, final):
+    return f"{nvars};\n{len(flines)};\n" + "".join(f + ";\n" for f in flines) + final + ";\n|"
+
+
+def one_sector(texts, **kw):
+    return SectorText(sector_id=kw.pop("sector_id", 0), texts=texts, **kw)
+
+
+# ------------------------------------------------------------------------------ A1: points
+
+@pytest.mark.parametrize("m,dim,first,count", [(13, 4, 0, 1000), (16, 4, 65000, 536), (21, 8, 12345, 777),
+                                               (1, 1, 0, 2), (40, 12, (1 << 40) - 300, 300), (0, 3, 0, 1)])
+def test_lattice_integers_bit_exact(fb, ctx, m, dim, first, count):
+    n_l = 1 << m
+    a = (0x9E3779B97F4A7C15 % n_l) | 1 if m > 0 else 1
+    rule = fb.Rule(kind=fb.RULE_LATTICE, n_shifts=3, korobov_a=a)
+    gv = OP.korobov_genvec(a % n_l if m > 0 else 0, n_l, dim) if m > 0 else [0] * dim
+    if m == 0:
+        rule.genvec = gv
+    for r in (0, 2):
+        t = ctx.generate_points(rule, 20151111, 7, r, n_l, first, count, dim)
+        delta = OP.lattice_shift(20151111, 7, r, dim)
+        ref = OP.lattice_t(np.arange(first, first + count, dtype=np.uint64), gv, n_l, delta)
+        assert np.array_equal(t, ref)
+
+
+@pytest.mark.parametrize("dim,first,count,it", [(1, 0, 100, 0), (7, (1 << 33) + 5, 1001, 3), (12, 0, 513, 1048575)])
+def test_philox_integers_bit_exact(fb, ctx, dim, first, count, it):
+    rule = fb.Rule(kind=fb.RULE_MC)
+    seed = 0xDEADBEEF12345678
+    t = ctx.generate_points(rule, seed, 123456, it, 0, first, count, dim)
+    ref = OP.philox_t(seed, 123456, OP.TAG_MC, it, np.arange(first, first + count, dtype=np.uint64), dim)
+    assert np.array_equal(t, ref)
+
+
+@pytest.mark.parametrize("r", [0, 1, 2, 3, 4, 5, 6])
+def test_periodising_transform(fb, ctx, r):
+    rng = np.random.default_rng(r)
+    t = rng.integers(0, 1 << 63, size=(4001, 5), dtype=np.uint64) * np.uint64(2) + np.uint64(1)
+    # the faces: u -> 0 and u -> 1
+    t[0, :] = 0
+    t[1, :] = np.uint64(0xFFFFFFFFFFFFFFFF)
+    t[2, :] = np.uint64(1) << np.uint64(63)
+    rule = fb.Rule(kind=fb.RULE_LATTICE, periodize_r=r)
+    x, xbar, w = ctx.transform_points(rule, t)
+    xo, xbo, wo = OP.korobov_transform(OP.unit_from_t(t), r)
+    wo = np.prod(wo, axis=1)
+    # x and 1-x each carry full relative accuracy at both faces (R4)
+    assert np.max(np.abs(x - xo.astype(float)) / xo.astype(float)) < 4e-15
+    assert np.max(np.abs(xbar - xbo.astype(float)) / xbo.astype(float)) < 4e-15
+    ok = wo.astype(float) > 1e-290          # u = 2^-53 underflows FP64 for r >= 5
+    assert np.max(np.abs(w[ok] - wo[ok].astype(float)) / wo[ok].astype(float)) < 2e-14
+
+
+def test_mc_transform_is_identity(fb, ctx):
+    rng = np.random.default_rng(5)
+    t = rng.integers(0, 1 << 63, size=(100, 3), dtype=np.uint64)
+    x, xbar, w = ctx.transform_points(fb.Rule(kind=fb.RULE_MC), t)
+    assert np.array_equal(x, OP.unit_from_t(t).astype(float))
+    assert np.all(w == 1.0)
+
+
+# ------------------------------------------------------------------------------ A5: program walk
+
+def _eval_case(ctx, wl, nsec, npts, seed):
+    prog = ctx.compile(wl.sectors, wl.dim)
+    rng = np.random.default_rng(seed)
+    x = rng.random((npts, wl.dim))
+    # points near the faces of the cube, where the integrands vary fastest
+    x[: wl.dim] = 0.5
+    for k in range(wl.dim):
+        x[k, k] = 1e-9
+    worst = 0.0
+    for si in range(nsec):
+        got = ctx.eval_points(prog, si, x)
+        ref, mag = oracle_values_and_magnitude(spec(wl.sectors[si]), x)
+        worst = max(worst, check_points(got, ref, mag))
+    prog.close()
+    return worst
+
+
+@pytest.mark.parametrize("name,nsec,npts", [("C1", 1, 2000), ("C2", 6, 1537), ("C3", 4, 1025), ("C4", 4, 700),
+                                            ("C5", 4, 999)])
+def test_per_point_parity_configs(ctx, name, nsec, npts):
+    wl = make_workload(name, nsectors=nsec, npoints=1 << 12)
+    assert _eval_case(ctx, wl, nsec, npts, 11) <= 1.0
+
+
+@pytest.mark.parametrize("npts", [1, 3, 511, 512, 513])
+def test_per_point_ragged_counts(ctx, npts):
+    wl = make_workload("C2", nsectors=1, npoints=1 << 12)
+    assert _eval_case(ctx, wl, 1, npts, npts) <= 1.0
+
+
+def test_eval_zero_points(ctx):
+    wl = make_workload("C1", nsectors=1, npoints=1 << 12)
+    prog = ctx.compile(wl.sectors, wl.dim)
+    assert ctx.eval_points(prog, 0, np.zeros((0, wl.dim))).shape == (0, 3)
+
+
+# ------------------------------------------------------------------------------ A6/A7: sums
+
+@pytest.mark.parametrize("name,nsec,npts,nsh", [("C1", 1, 1 << 16, 1), ("C1", 1, 1 << 16, 8), ("C2", 3, 1 << 15, 1),
+                                                ("C3", 2, 1 << 15, 8), ("C4", 2, 1 << 14, 1), ("C4", 2, 1 << 14, 4)])
+def test_lattice_partial_sums_parity(fb, ctx, name, nsec, npts, nsh):
+    wl = make_workload(name, nsectors=nsec, npoints=npts, n_shifts=nsh)
+    prog = ctx.compile(wl.sectors, wl.dim)
+    rule = fb.Rule.from_workload(wl)
+    gpu = ctx.partial_sums(prog, wl.npoints, rule, wl.seed)
+    gv = genvec_of(wl)
+    for si in range(nsec):
+        s1, s2, sa = OI.lattice_partial_sums(spec(wl.sectors[si]), wl.n_lattice, wl.n_shifts, gv, wl.periodize_r, wl.seed)
+        check_sums(gpu[si], s1, s2, sa)
+    # the estimator (R5) on the device against the oracle's, from the oracle's own sums
+    res = ctx.integrate(prog, wl.npoints, rule, wl.seed)
+    for si in range(nsec):
+        val, sig = OI.integrate_lattice(spec(wl.sectors[si]), wl.npoints, wl.n_shifts, gv, wl.periodize_r, wl.seed)[:2]
+        val, sig = np.asarray(val, dtype=float), np.asarray(sig, dtype=float)
+        assert np.allclose(res[si]["re"], val[:, 0], rtol=1e-9, atol=1e-13 * np.abs(val).max())
+        assert np.allclose(res[si]["re_err"], sig[:, 0], rtol=1e-5, atol=1e-12 * np.abs(val).max())
+        if val.shape[1] == 2:
+            assert np.allclose(res[si]["im"], val[:, 1], rtol=1e-9, atol=1e-13 * np.abs(val).max())
+            assert np.allclose(res[si]["im_err"], sig[:, 1], rtol=1e-5, atol=1e-12 * np.abs(val).max())
+        assert np.all(res[si]["neval"] == wl.npoints) and np.all(res[si]["n_nonfinite"] == 0)
+
+
+def test_sector_selection_and_order(fb, ctx):
+    """sectors=[2,0] integrates those two, in that order, with streams keyed by sector_id."""
+    wl = make_workload("C2", nsectors=3, npoints=1 << 12)
+    prog = ctx.compile(wl.sectors, wl.dim)
+    rule = fb.Rule.from_workload(wl)
+    full = ctx.partial_sums(prog, wl.npoints, rule, wl.seed)
+    sub = ctx.partial_sums(prog, wl.npoints, rule, wl.seed, sectors=[2, 0])
+    assert np.allclose(sub[0], full[2], rtol=1e-13) and np.allclose(sub[1], full[0], rtol=1e-13)
+
+
+@pytest.mark.parametrize("npts", [2, 10007, (1 << 17) + 3])
+def test_mc_sums_ragged(fb, ctx, npts):
+    """Plain MC (Philox) with point counts that are not multiples of the block's work quantum."""
+    wl = make_workload("C1", nsectors=1, npoints=1 << 12)
+    prog = ctx.compile(wl.sectors, wl.dim)
+    rule = fb.Rule(kind=fb.RULE_MC)
+    sec = spec(wl.sectors[0])
+    gpu = ctx.partial_sums(prog, npts, rule, 99)[0, 0]          # [K,1,2]
+    s1 = np.zeros((sec.K, 1), dtype=LD)
+    s2 = np.zeros((sec.K, 1), dtype=LD)
+    for first in range(0, npts, 1 << 14):
+        cnt = min(1 << 14, npts - first)
+        _, x = OI.mc_points(sec, 99, 0, first, cnt)
+        v = OI.integrand_values(sec, x)
+        s1[:, 0] += np.sum(v, axis=1)
+        s2[:, 0] += np.sum(v * v, axis=1)
+    assert np.allclose(gpu[..., 0], s1.astype(float), rtol=1e-10)
+    assert np.allclose(gpu[..., 1], s2.astype(float), rtol=1e-10)
+    val, sig = OI.integrate_mc(sec, npts, 99)[:2]
+    res = ctx.integrate(prog, npts, rule, 99)[0]
+    assert np.allclose(res["re"], np.asarray(val, dtype=float)[:, 0], rtol=1e-9)
+    assert np.allclose(res["re_err"], np.asarray(sig, dtype=float)[:, 0], rtol=1e-5)
+
+
+# ------------------------------------------------------------------------------ closed forms (4 sigma)
+
+def _within(res, exact, nsig=4.0):
+    return abs(res["re"] - exact) <= nsig * res["re_err"] + 1e-15 * abs(exact)
+
+
+def test_paper_worker_example(fb, ctx):
+    """`1; 0; x[1]+0.2;` integrates to 0.7."""
+    sec = one_sector(["1;\n0;\nx[1]+0.2;\n|"])
+    prog = ctx.compile([sec], 1)
+    res = ctx.integrate(prog, 8 << 10, fb.Rule(kind=fb.RULE_LATTICE, n_shifts=8, korobov_a=1, periodize_r=3), 1)[0, 0]
+    assert _within(res, 0.7) and res["re_err"] < 1e-6
+    res = ctx.integrate(prog, 1 << 20, fb.Rule(kind=fb.RULE_MC), 1)[0, 0]
+    assert _within(res, 0.7) and res["re_err"] < 1e-3
+
+
+def test_monomial_closed_form(fb, ctx):
+    """BASELINE C1's closed-form check: int prod x_i^a_i over [0,1]^4 = prod 1/(a_i+1)."""
+    from workloads import korobov_a
+    a = [2, 0, 1, 2]
+    txt = block(4, [], "*".join(f"p[x[{i + 1}],{e}]" for i, e in enumerate(a) if e) + "*1.0")
+    sec = one_sector([txt])
+    prog = ctx.compile([sec], 4)
+    exact = float(np.prod([1.0 / (e + 1) for e in a]))
+    bad = 0
+    for seed in range(20):
+        rule = fb.Rule(kind=fb.RULE_LATTICE, n_shifts=8, korobov_a=korobov_a(1 << 13, 4), periodize_r=3)
+        res = ctx.integrate(prog, 1 << 16, rule, seed)[0, 0]
+        bad += not _within(res, exact)
+        assert res["re_err"] < 1e-5 * exact
+    assert bad <= 1
+
+
+def test_noninteger_power_closed_form(fb, ctx):
+    """int prod x_i^-0.4 = (1/0.6)^3 with the MC rule and with Vegas (a >= -0.45: finite variance)."""
+    sec = one_sector([block(3, [], "p[x[1],-0.4]*p[x[2],-0.4]*p[x[3],-0.4]")])
+    prog = ctx.compile([sec], 3)
+    exact = (1 / 0.6) ** 3
+    res = ctx.integrate(prog, 1 << 20, fb.Rule(kind=fb.RULE_MC), 3)[0, 0]
+    assert _within(res, exact) and res["re_err"] < 0.01
+    res = ctx.integrate(prog, 1 << 17, fb.Rule(kind=fb.RULE_VEGAS, vegas_bins=50, vegas_iters=10), 3)[0, 0]
+    assert _within(res, exact, 5.0) and res["re_err"] < 0.002
+
+
+def test_bubble_eps_orders(fb, ctx):
+    """One-loop massless bubble (eq. 2): twice the order-k integral = c_k (golden file)."""
+    from conftest import golden
+    g = golden("bubble_eps_coefficients.txt")
+    fl = ["1+x[1]", "2*l[f[1]]-l[x[1]]"]
+    fact = [1, 1, 2, 6, 24]
+    texts = [block(1, fl, f"2*p[f[1],-2]*p[f[2],{k}]/{fact[k]}" if k else "2*p[f[1],-2]") for k in range(5)]
+    prog = ctx.compile([one_sector(texts)], 1)
+    res = ctx.integrate(prog, 8 << 13, fb.Rule(kind=fb.RULE_LATTICE, n_shifts=8, korobov_a=1, periodize_r=3), 5)[0]
+    for k in range(5):
+        exact = float(g[f"c{k}"])
+        assert _within(res[k], exact), (k, res[k], exact)
+        assert abs(res[k]["re"] - exact) < 1e-9
+
+
+def test_contour_1d_closed_forms(fb, ctx):
+    """F = x - a, z = x - i lam x(1-x): int dz/(z-a), int log(z-a) dz, int (z-a)^-1/2 dz (golden file)."""
+    from conftest import golden
+    g = golden("contour_1d_closed_forms.txt")
+    texts = [block(1, ["x[1]-0.3"], f) for f in ("1/f[1]", "l[f[1]]", "p[f[1],-0.5]")]
+    sec = one_sector(texts, is_complex=True, deform_f_index=1, lam=0.5)
+    prog = ctx.compile([sec], 1)
+    res = ctx.integrate(prog, 8 << 13, fb.Rule(kind=fb.RULE_LATTICE, n_shifts=8, korobov_a=1, periodize_r=3), 5)[0]
+    for k, key in enumerate(("inv", "log", "rsqrt")):
+        re, im = float(g[key + "_re"]), float(g[key + "_im"])
+        assert abs(res[k]["re"] - re) <= 4 * res[k]["re_err"] + 1e-14
+        assert abs(res[k]["im"] - im) <= 4 * res[k]["im_err"] + 1e-14
+        assert abs(res[k]["re"] - re) < 1e-8 and abs(res[k]["im"] - im) < 1e-8
+
+
+def test_lambda_zero_reproduces_real_path(fb, ctx):
+    """R11: at lambda = 0 the complex path gives the real path's values with Im = 0."""
+    wl = make_workload("C4", nsectors=1, npoints=1 << 12)
+    s = wl.sectors[0]
+    real = SectorText(s.sector_id, s.texts)
+    zero = SectorText(s.sector_id, s.texts, is_complex=True, deform_f_index=s.deform_f_index, lam=0.0)
+    prog = ctx.compile([real, zero], wl.dim)
+    x = np.random.default_rng(2).random((500, wl.dim))
+    a, b = ctx.eval_points(prog, 0, x), ctx.eval_points(prog, 1, x)
+    ok = np.isfinite(a.real)            # F changes sign inside the cube: the real path has NaNs there
+    assert ok.sum() > 100
+    assert np.allclose(b.real[ok], a.real[ok], rtol=1e-11) and np.all(np.abs(b.imag[ok]) <= 1e-11 * np.abs(a.real[ok]))
+
+
+# ------------------------------------------------------------------------------ A3/A8: Vegas
+
+def _c5(nsec, npts):
+    return make_workload("C5", nsectors=nsec, npoints=npts)
+
+
+def test_vegas_iteration_stepwise(fb, ctx):
+    """Same grid in => sums match (R15) and the f^2 histogram matches bin by bin (pin vi)."""
+    wl = _c5(2, 20000)
+    prog = ctx.compile(wl.sectors, wl.dim)
+    rule = fb.Rule.from_workload(wl)
+    rng = np.random.default_rng(8)
+    for si, it in ((0, 0), (1, 3)):
+        sec = spec(wl.sectors[si])
+        if it == 0:
+            grid = OI.vegas_uniform_grid(wl.dim, wl.vegas_bins)
+        else:  # an uneven but valid grid
+            w = rng.random((wl.dim, wl.vegas_bins)).astype(LD) ** 3 + LD(1e-3)
+            grid = np.concatenate([np.zeros((wl.dim, 1), dtype=LD), np.cumsum(w, axis=1) / np.sum(w, axis=1)[:, None]], axis=1)
+            grid[:, -1] = 1
+        gridf = grid.astype(np.float64)
+        s1, s2, hist = OI.vegas_iteration_sums(sec, gridf.astype(LD), wl.npoints, wl.seed, it)
+        sums, h = ctx.vegas_iteration(prog, si, wl.npoints, rule, wl.seed, it, gridf)
+        assert np.allclose(sums[..., 0], s1.astype(float), rtol=1e-10)
+        assert np.allclose(sums[..., 1], s2.astype(float), rtol=1e-10)
+        hf = hist.astype(float)
+        assert np.allclose(h, hf, rtol=1e-10, atol=1e-13 * hf.max())
+        # pin iii: every dimension's histogram has the same total, the deterministic sum of g^2
+        assert np.allclose(h.sum(axis=1), sums[0, 0, 1], rtol=1e-12)
+
+
+def test_vegas_refine_parity(fb, ctx):
+    """Same histogram in => edges match to 1e-13 (pin vi); invariants (pin ii); flat in => uniform out."""
+    rng = np.random.default_rng(9)
+    nb = 50
+    grids, hists = [], []
+    for i in range(40):
+        w = rng.random(nb) ** 2 + 1e-3
+        g = np.concatenate([[0.0], np.cumsum(w) / np.sum(w)])
+        g[-1] = 1.0
+        h = rng.random(nb) ** (1 + i % 5) * 10.0 ** rng.integers(-8, 8)
+        if i % 7 == 0:
+            h[rng.integers(0, nb, 10)] = 0.0       # empty bins
+        if i == 5:
+            h[:] = 0.0                              # nothing sampled: grid must stay
+        if i == 6:
+            h[:] = 0.0
+            h[17] = 1.0                             # a single hot bin
+        grids.append(g)
+        hists.append(h)
+    grids, hists = np.array(grids), np.array(hists)
+    out = ctx.vegas_refine(grids, hists, 1.5)
+    for i in range(40):
+        ref = OI.vegas_refine(grids[i].astype(LD), hists[i].astype(LD), 1.5).astype(float)
+        assert np.max(np.abs(out[i] - ref)) < 1e-13, i
+        assert out[i][0] == 0.0 and out[i][-1] == 1.0 and np.all(np.diff(out[i]) > 0)
+    uni = np.arange(nb + 1) / nb
+    out = ctx.vegas_refine(uni[None, :], np.full((1, nb), 3.0), 1.5)
+    assert np.max(np.abs(out[0] - uni)) < 1e-15
+    for nb2 in (2, 3, 128):
+        uni = np.arange(nb2 + 1) / nb2
+        h = rng.random(nb2)
+        ref = OI.vegas_refine(uni.astype(LD), h.astype(LD), 0.7).astype(float)
+        assert np.max(np.abs(ctx.vegas_refine(uni[None, :], h[None, :], 0.7)[0] - ref)) < 1e-13
+
+
+def test_vegas_full_run_against_oracle(fb, ctx):
+    """10 iterations: the histogram is summed by atomics in no fixed order, so grids agree to
+    rounding only and the final numbers to ~1e-9 (points near a bin edge may change bins)."""
+    wl = _c5(2, 1 << 13)
+    prog = ctx.compile(wl.sectors, wl.dim)
+    rule = fb.Rule.from_workload(wl)
+    res = ctx.integrate(prog, wl.npoints, rule, wl.seed)
+    for si in range(2):
+        val, sig, chi2, grid = OI.integrate_vegas(spec(wl.sectors[si]), wl.npoints, wl.seed, wl.vegas_bins, wl.vegas_iters,
+                                                  wl.vegas_alpha)
+        g, h = ctx.vegas_grid(si, wl.dim, wl.vegas_bins)
+        assert np.max(np.abs(g - grid.astype(float))) < 1e-9
+        assert g[:, 0].max() == 0.0 and g[:, -1].min() == 1.0 and np.all(np.diff(g, axis=1) > 0)
+        assert np.isclose(res[si, 0]["re"], float(val[0, 0]), rtol=1e-7)
+        assert np.isclose(res[si, 0]["re_err"], float(sig[0, 0]), rtol=1e-5)
+        assert np.isclose(res[si, 0]["chi2"], float(chi2[0, 0]), rtol=1e-4, atol=1e-6)
+        assert res[si, 0]["neval"] == wl.npoints * wl.vegas_iters
+
+
+def test_vegas_constant_integrand(fb, ctx):
+    """Pin i: f = 1 gives I = 1 exactly with sigma_it = 0 in iteration 1, and stays 1 within rounding."""
+    prog = ctx.compile([one_sector([block(3, [], "1.0+0*x[1]")])], 3)
+    res = ctx.integrate(prog, 1 << 14, fb.Rule(kind=fb.RULE_VEGAS, vegas_bins=50, vegas_iters=1), 4)[0, 0]
+    assert res["re"] == 1.0 and res["re_err"] == 0.0
+    res = ctx.integrate(prog, 1 << 14, fb.Rule(kind=fb.RULE_VEGAS, vegas_bins=50, vegas_iters=5), 4)[0, 0]
+    assert abs(res["re"] - 1.0) <= 4 * res["re_err"] + 1e-12
+
+
+def test_vegas_adapts_to_separable_peak(fb, ctx):
+    """Pin v: f = prod (1-a) x^-a, a = 0.4: edges move towards (b/NB)^(1/(1-a)); the error shrinks."""
+    sec = one_sector([block(2, [], "0.36*p[x[1],-0.4]*p[x[2],-0.4]")])
+    prog = ctx.compile([sec], 2)
+    r1 = ctx.integrate(prog, 1 << 16, fb.Rule(kind=fb.RULE_VEGAS, vegas_bins=50, vegas_iters=1), 6)[0, 0]
+    r10 = ctx.integrate(prog, 1 << 16, fb.Rule(kind=fb.RULE_VEGAS, vegas_bins=50, vegas_iters=10), 6)[0, 0]
+    g, _ = ctx.vegas_grid(0, 2, 50)
+    ideal = (np.arange(51) / 50) ** (1 / 0.6)
+    assert np.max(np.abs(g - ideal[None, :])) < 0.02
+    assert r10["re_err"] < 0.3 * r1["re_err"] and abs(r10["re"] - 1.0) <= 4 * r10["re_err"]
+
+
+# ------------------------------------------------------------------------------ limits and errors
+
+def test_max_dim_and_max_orders(fb, ctx):
+    """dim = 12 (FIESTA_MAX_DIM) and K = 8 (FIESTA_MAX_ORDERS) in one sector."""
+    fl = ["1+" + "+".join(f"{0.1 * (i + 1):.1f}*x[{i + 1}]" for i in range(12)), "l[f[1]]"]
+    texts = [block(12, fl, f"p[f[1],-{k + 1}]*p[f[2],{k}]*x[12]*x[1]" if k else "p[f[1],-1]*x[12]*x[1]") for k in range(8)]
+    sec = one_sector(texts, sector_id=41)
+    prog = ctx.compile([sec], 12)
+    x = np.random.default_rng(3).random((600, 12))
+    ref, mag = oracle_values_and_magnitude(spec(sec), x)
+    assert check_points(ctx.eval_points(prog, 0, x), ref, mag) <= 1.0
+    rule = fb.Rule(kind=fb.RULE_LATTICE, n_shifts=2, korobov_a=1571, periodize_r=2)
+    gpu = ctx.partial_sums(prog, 1 << 13, rule, 17)
+    s1, s2, sa = OI.lattice_partial_sums(spec(sec), 1 << 12, 2, OP.korobov_genvec(1571, 1 << 12, 12), 2, 17)
+    check_sums(gpu[0], s1, s2, sa)
+
+
+def test_many_temporaries_spill_to_shared(fb, ctx):
+    """More live f[i] than register temporaries: compiler-directed shared-memory slots (n_mem_slots > 0)."""
+    nf = 14
+    fl = [f"1+{0.3 + 0.1 * i:.1f}*x[{i % 3 + 1}]+x[{(i + 1) % 3 + 1}]*x[{(i + 2) % 3 + 1}]" for i in range(nf)]
+    final = "+".join(f"l[f[{i + 1}]]*p[f[{(i + 5) % nf + 1}],-1.5]" for i in range(nf))
+    sec = one_sector([block(3, fl, final)])
+    prog = ctx.compile([sec], 3)
+    assert prog.info[0]["n_mem_slots"] > 0
+    x = np.random.default_rng(4).random((300, 3))
+    ref, mag = oracle_values_and_magnitude(spec(sec), x)
+    assert check_points(ctx.eval_points(prog, 0, x), ref, mag) <= 1.0
+    gpu = ctx.partial_sums(prog, 1 << 12, fb.Rule(kind=fb.RULE_LATTICE, korobov_a=1, periodize_r=1, genvec=[1, 433, 1217]), 2)
+    s1, s2, sa = OI.lattice_partial_sums(spec(sec), 1 << 12, 1, [1, 433, 1217], 1, 2)
+    check_sums(gpu[0], s1, s2, sa)
+
+
+def test_constants_and_operators(fb, ctx):
+    """Grammar coverage: P, G, PolyGamma, unary minus, division, nested p[], l[]."""
+    final = ("P*x[1]-G*x[2]+PolyGamma[2,1]*x[1]*x[2]-(-x[1]+2)/(1+x[2])+p[1+x[1]*x[2],3]/p[2+x[1],2]"
+             "+l[1+p[x[2],2]]*p[1+x[1],0.5]-p[1+x[2],-1.5]+1.5e-3*x[1]-p[l[2+x[1]],2]")
+    sec = one_sector([block(2, [], final)])
+    prog = ctx.compile([sec], 2)
+    x = np.random.default_rng(5).random((400, 2))
+    ref, mag = oracle_values_and_magnitude(spec(sec), x)
+    assert check_points(ctx.eval_points(prog, 0, x), ref, mag) <= 1.0
+
+
+def test_nonfinite_is_reported(fb, ctx):
+    """R13: l[e] with e <= 0 in real mode is NaN, counted, and raises FIESTA_E_NONFINITE."""
+    prog = ctx.compile([one_sector([block(1, [], "l[x[1]-0.5]")])], 1)
+    with pytest.raises(fb.FiestaError) as ei:
+        ctx.integrate(prog, 1 << 10, fb.Rule(kind=fb.RULE_MC), 1)
+    assert ei.value.code == -6
+    res = ctx.integrate(prog, 1 << 10, fb.Rule(kind=fb.RULE_MC), 1, allow_nonfinite=True)[0, 0]
+    t = ctx.generate_points(fb.Rule(kind=fb.RULE_MC), 1, 0, 0, 0, 0, 1 << 10, 1)
+    assert res["n_nonfinite"] == int(np.sum(OP.unit_from_t(t) < 0.5))
+
+
+@pytest.mark.parametrize("text,dim,code", [
+    ("1;\n0;\nx[1]+;\n|", 1, -1), ("1;\n0;\nx[1]+0.2;\n", 1, -1), ("1;\n0;\nq[1];\n|", 1, -1),
+    ("1;\n0;\nx[2];\n|", 1, -2), ("1;\n1;\nx[1];\nf[2];\n|", 1, -1), ("1;\n0;\nPolyGamma[9,9];\n|", 1, -1),
+    ("1;\n0;\np[x[1],x[1]];\n|", 1, -1), ("13;\n0;\nx[1];\n|", 13, -2)])
+def test_compile_errors(fb, ctx, text, dim, code):
+    with pytest.raises(fb.FiestaError) as ei:
+        ctx.compile([one_sector([text])], dim)
+    assert ei.value.code == code, str(ei.value)
+
+
+def test_deformation_needs_polynomial(fb, ctx):
+    sec = one_sector([block(1, ["l[1+x[1]]"], "f[1]")], is_complex=True, deform_f_index=1, lam=0.5)
+    with pytest.raises(fb.FiestaError) as ei:
+        ctx.compile([sec], 1)
+    assert ei.value.code == -3
+
+
+def test_rule_errors(fb, ctx):
+    prog = ctx.compile([one_sector([block(1, [], "x[1]")])], 1)
+    for npts, rule in [(1000, fb.Rule(kind=0)), (1 << 10, fb.Rule(kind=0, n_shifts=3)), (1 << 10, fb.Rule(kind=0, periodize_r=7)),
+                       (1 << 10, fb.Rule(kind=2, vegas_bins=1)), (1 << 10, fb.Rule(kind=2, vegas_bins=129)), (1 << 10, fb.Rule(kind=5)),
+                       (1, fb.Rule(kind=1)), (1 << 10, fb.Rule(kind=0, genvec=[1 << 10]))]:
+        with pytest.raises(fb.FiestaError) as ei:
+            ctx.integrate(prog, npts, rule, 1)
+        assert ei.value.code == -4, (npts, rule, str(ei.value))
+
+
+# ------------------------------------------------------------------------------ full sizes, bench launch configuration
+
+def test_c2_full_size_sampled_sectors(fb, ctx):
+    """BASELINE config 2 at full size (64 sectors x 2^20 points, one launch): the sums of two
+    sampled sectors against the oracle, every sector's result finite with no bad point."""
+    wl = make_workload("C2")
+    prog = ctx.compile(wl.sectors, wl.dim)
+    rule = fb.Rule.from_workload(wl)
+    gpu = ctx.partial_sums(prog, wl.npoints, rule, wl.seed)
+    gv = genvec_of(wl)
+    for si in (5, 63):
+        s1, s2, sa = OI.lattice_partial_sums(spec(wl.sectors[si]), wl.n_lattice, 1, gv, wl.periodize_r, wl.seed)
+        check_sums(gpu[si], s1, s2, sa)
+    res = ctx.integrate(prog, wl.npoints, rule, wl.seed)
+    assert res.shape == (64, 4) and np.all(res["n_nonfinite"] == 0) and np.all(np.isfinite(res["re"]))
+    assert np.allclose(res["re"], gpu[:, 0, :, 0, 0] / wl.npoints, rtol=1e-12)
+
+
+def test_c3_bench_configuration_sampled(fb, ctx):
+    """The workload bench.py times (config 3: dim 8, K = 5, 8 shifts x 2^21 points per sector,
+    16 chunks per (sector, shift)) on a slice of its sectors: one sampled (sector, shift) sum
+    against the oracle, and the properties that hold at any size -- per-shift sums agree with
+    each other to the quoted error, results are finite, neval is exact."""
+    wl = make_workload("C3", nsectors=6)
+    assert wl.npoints == 1 << 24 and wl.n_shifts == 8
+    prog = ctx.compile(wl.sectors, wl.dim)
+    rule = fb.Rule.from_workload(wl)
+    gpu = ctx.partial_sums(prog, wl.npoints, rule, wl.seed)          # [6, 8, 5, 1, 2]
+    si, r = 4, 6
+    s1, s2, sa = OI.lattice_partial_sums(spec(wl.sectors[si]), wl.n_lattice, 8, genvec_of(wl), wl.periodize_r, wl.seed,
+                                         shifts=[r])
+    check_sums(gpu[si, r:r + 1], s1[r:r + 1], s2[r:r + 1], sa[r:r + 1])
+    res = ctx.integrate(prog, wl.npoints, rule, wl.seed)
+    assert np.all(res["neval"] == 1 << 24) and np.all(res["n_nonfinite"] == 0)
+    q = gpu[..., 0, 0] / wl.n_lattice                                   # [6, 8, 5]
+    assert np.allclose(res["re"], q.mean(axis=1), rtol=1e-12)
+    assert np.allclose(res["re_err"], q.std(axis=1, ddof=1) / np.sqrt(8), rtol=1e-6)
+    assert np.all(np.abs(q - q.mean(axis=1, keepdims=True)) <= 6 * q.std(axis=1, ddof=1, keepdims=True) + 1e-300)
+
+
+def test_fp64_peak_is_plausible(ctx):
+    """The roofline denominator: DFMA streams on every SM.  B200: 148 SM x 64 lanes x 2 x 1.965 GHz = 37.2."""
+    t = ctx.fp64_peak(50.0)
+    assert 15.0 < t < 45.0

@@ -1,0 +1,135 @@
+"""CPU-only tests of the host side: the C-ABI library loads and exports every declared symbol,
+the host-arithmetic entry point fiesta_combine, no-GPU failure is loud, and the multi-GPU
+sharding logic (world_size 2 over gloo).  No compute calls on a device here."""
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol(lib):
+    hdr = open(os.path.join(ROOT, "include", "fiesta_b200.h")).read()
+    declared = set(re.findall(r"\b(fiesta_[a-z0-9_]+)\s*\(", hdr))
+    assert len(declared) >= 19
+    handle = lib.load_library()
+    for name in declared:
+        assert getattr(handle, name) is not None, name
+    assert declared == set(lib.exported_symbols())
+    out = subprocess.run(["nm", "-D", "--defined-only", lib.LIB_PATH], capture_output=True, text=True).stdout
+    exported = set(re.findall(r" T (fiesta_[a-z0-9_]+)", out))
+    assert declared <= exported
+
+
+def test_library_is_built_for_sm100a(lib):
+    out = subprocess.run(["cuobjdump", "-lelf", lib.LIB_PATH], capture_output=True, text=True).stdout
+    assert "sm_100a" in out and "sm_90" not in out
+
+
+def test_struct_layouts_match_header(lib):
+    assert lib.RESULT_DTYPE.itemsize == 56      # 5 doubles + 2 uint64
+    assert lib.INFO_DTYPE.itemsize == 48        # 9 int32 (+pad) + 1 double
+
+
+def test_combine_mean_square(lib):
+    """values add, errors add in mean square."""
+    rng = np.random.default_rng(0)
+    S, K = 7, 3
+    per = np.zeros((S, K), dtype=lib.RESULT_DTYPE)
+    for f in ("re", "re_err", "im", "im_err", "chi2"):
+        per[f] = rng.random((S, K))
+    per["neval"] = 100
+    per["n_nonfinite"] = rng.integers(0, 3, (S, K))
+    tot = np.zeros(K, dtype=lib.RESULT_DTYPE)
+    from paper_1511_03614_b200.binding import _ptr
+    rc = lib.load_library().fiesta_combine(_ptr(per), S, K, _ptr(tot))
+    assert rc == 0
+    assert np.allclose(tot["re"], per["re"].sum(axis=0), rtol=1e-15)
+    assert np.allclose(tot["im"], per["im"].sum(axis=0), rtol=1e-15)
+    assert np.allclose(tot["re_err"], np.sqrt((per["re_err"] ** 2).sum(axis=0)), rtol=1e-15)
+    assert np.allclose(tot["im_err"], np.sqrt((per["im_err"] ** 2).sum(axis=0)), rtol=1e-15)
+    assert np.all(tot["neval"] == 100 * S) and np.all(tot["n_nonfinite"] == per["n_nonfinite"].sum(axis=0))
+    assert lib.load_library().fiesta_combine(None, S, K, _ptr(tot)) == -7
+
+
+def test_no_gpu_fails_loudly(lib):
+    """No CPU fallback: without an sm_100 device the context cannot be created."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    with pytest.raises(lib.FiestaError) as ei:
+        lib.Context(0)
+    assert ei.value.code == -5
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_1511_03614_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cpp", ".cu", ".cuh", ".h", ".hpp", ".inc")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle\b", text, re.M), f
+                assert "oracle/" not in text, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith(".py"):
+            assert "paper_1511_03614_b200" not in open(os.path.join(ROOT, "oracle", f)).read().replace(
+                "`paper_1511_03614_b200/`", ""), f
+
+
+# ------------------------------------------------------------------------------ sharding
+
+def test_partition_is_balanced_and_complete():
+    from paper_1511_03614_b200.sharding import partition_sectors
+    rng = np.random.default_rng(1)
+    costs = rng.integers(500, 1500, 2000).astype(float)
+    for world in (1, 2, 3, 8):
+        parts = partition_sectors(costs, world)
+        allidx = sorted(i for p in parts for i in p)
+        assert allidx == list(range(2000))
+        loads = [costs[p].sum() for p in parts]
+        assert max(loads) - min(loads) <= costs.max()
+    assert partition_sectors([5.0], 4) == [[0], [], [], []]
+    assert partition_sectors([], 2) == [[], []]
+
+
+_GLOO_WORKER = r"""
+import os, sys
+import numpy as np
+import torch.distributed as dist
+sys.path.insert(0, {root!r})
+from paper_1511_03614_b200.sharding import partition_sectors, gather_results, max_over_ranks
+from paper_1511_03614_b200.binding import RESULT_DTYPE
+dist.init_process_group("gloo", init_method="tcp://127.0.0.1:{port}", rank=int(sys.argv[1]), world_size=2)
+rank = dist.get_rank()
+S, K = 11, 3
+costs = [(i * 7) % 5 + 1 for i in range(S)]
+mine = partition_sectors(costs, 2)[rank]
+local = np.zeros((len(mine), K), dtype=RESULT_DTYPE)
+for a, s in enumerate(mine):          # a stand-in for this rank's fiesta_integrate output
+    for k in range(K):
+        local[a, k] = (s + 0.1 * k, 0.01 * s, -s, 0.5, k, 1000 + s, s % 2)
+full = gather_results(local, mine, S, dist)
+for s in range(S):
+    for k in range(K):
+        assert full[s, k]["re"] == s + 0.1 * k and full[s, k]["neval"] == 1000 + s and full[s, k]["im"] == -s
+t = max_over_ranks(1.0 + rank, dist)
+assert t == 2.0
+dist.barrier()
+dist.destroy_process_group()
+print("ok", rank)
+"""
+
+
+def test_gather_results_world_size_2_gloo(tmp_path):
+    port = 29500 + (os.getpid() % 2000)
+    script = tmp_path / "worker.py"
+    script.write_text(_GLOO_WORKER.format(root=ROOT, port=port))
+    procs = [subprocess.Popen([sys.executable, str(script), str(r)], stdout=subprocess.PIPE, stderr=subprocess.STDOUT,
+                              text=True) for r in range(2)]
+    outs = [p.communicate(timeout=180)[0] for p in procs]
+    for r, (p, o) in enumerate(zip(procs, outs)):
+        assert p.returncode == 0 and f"ok {r}" in o, o
