@@ -46,6 +46,12 @@ def _run(cmd, log):
 
 def build(force=False, verbose=False):
     os.makedirs(OBJ, exist_ok=True)
+    gen_src = os.path.join(CSRC, "gen_interp_ptx.py")
+    gen_out = os.path.join(CSRC, "fx_interp_gen.inc")
+    if force or _stale(gen_out, [gen_src, os.path.join(CSRC, "fx_isa.h")]):
+        text = subprocess.run([sys.executable, gen_src], stdout=subprocess.PIPE, check=True, text=True).stdout
+        with open(gen_out, "w") as f:
+            f.write(text)
     hdrs = _deps()
     jobs = []  # (object, cmd, sources)
 
@@ -61,7 +67,7 @@ def build(force=False, verbose=False):
     for name in ("fiesta_abi", "fx_compiler"):
         o = os.path.join(OBJ, name + ".o")
         s = os.path.join(CSRC, name + ".cpp")
-        jobs.append((o, ["g++", "-O2", "-std=c++17", "-fPIC", "-I/usr/local/cuda/include", "-c", s, "-o", o],
+        jobs.append((o, ["g++", "-O2", "-std=c++17", "-fPIC", "-pthread", "-I/usr/local/cuda/include", "-c", s, "-o", o],
                      [s] + hdrs))
     todo = [(o, c) for (o, c, srcs) in jobs if force or _stale(o, srcs)]
     if verbose and todo:
@@ -70,7 +76,7 @@ def build(force=False, verbose=False):
         list(ex.map(lambda oc: _run(oc[1], oc[0] + ".log"), todo))
     objs = [o for (o, _, _) in jobs]
     if force or todo or _stale(LIB, objs):
-        _run([NVCC, "-shared", "-o", LIB] + ARCH + objs + ["-lcudart"], os.path.join(OBJ, "link.log"))
+        _run([NVCC, "-shared", "-o", LIB] + ARCH + objs + ["-lcudart", "-lpthread"], os.path.join(OBJ, "link.log"))
     return LIB
 
 

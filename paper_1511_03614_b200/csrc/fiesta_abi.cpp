@@ -4,6 +4,9 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <atomic>
+#include <mutex>
+#include <thread>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -176,43 +179,78 @@ int fiesta_compile(fiesta_ctx *ctx, const fiesta_sector_desc *sectors, int32_t n
   pg->device = ctx->device;
   pg->dim = dim;
   std::vector<fx_ins> arena;
-  try {
-    for (int s = 0; s < nsectors; ++s) {
-      const fiesta_sector_desc &d = sectors[s];
-      fx::CompiledSector cs;
-      try {
-        cs = fx::compile_sector(d.expr, d.n_orders, dim, d.is_complex != 0, d.deform_f_index, d.lambda);
-      } catch (fx::CompileError &e) {
-        e.msg = "sector " + std::to_string(s) + " (id " + std::to_string(d.sector_id) + "), " + e.msg;
-        throw;
+  // sectors are independent: parse/optimise them on the host cores in parallel, then lay the
+  // programs out in the arena in sector order
+  std::vector<fx::CompiledSector> compiled(nsectors);
+  {
+    std::atomic<int> next{0};
+    std::mutex err_mu;
+    int err_sector = nsectors;
+    fx::CompileError err{0, ""};
+    auto worker = [&]() {
+      for (;;) {
+        const int s = next.fetch_add(1);
+        if (s >= nsectors) return;
+        const fiesta_sector_desc &d = sectors[s];
+        try {
+          if (!d.expr || d.n_orders < 1 || d.n_orders > FIESTA_MAX_ORDERS)
+            throw fx::CompileError{FIESTA_E_ARG, "n_orders must be in 1..8 and expr non-NULL"};
+          compiled[s] = fx::compile_sector(d.expr, d.n_orders, dim, d.is_complex != 0, d.deform_f_index, d.lambda);
+          compiled[s].sector_id = d.sector_id;
+        } catch (fx::CompileError &e) {
+          std::lock_guard<std::mutex> g(err_mu);
+          if (s < err_sector) {
+            err_sector = s;
+            err = e;
+            err.msg = "sector " + std::to_string(s) + " (id " + std::to_string(d.sector_id) + "), " + e.msg;
+          }
+        } catch (std::exception &e) {
+          std::lock_guard<std::mutex> g(err_mu);
+          if (s < err_sector) {
+            err_sector = s;
+            err = fx::CompileError{FIESTA_E_ARG, std::string("sector ") + std::to_string(s) + ": " + e.what()};
+          }
+        }
       }
-      cs.sector_id = d.sector_id;
-      fx_sector_dev sd{};
-      fx_ins pad{};
-      pad.op = FX_END;
-      sd.main_off = (uint32_t)arena.size();
-      arena.insert(arena.end(), cs.main.begin(), cs.main.end());
-      arena.push_back(pad);
-      sd.main_len = (uint32_t)cs.main.size() + 1;
-      if (!cs.deform.empty()) {
-        sd.deform_off = (uint32_t)arena.size();
-        arena.insert(arena.end(), cs.deform.begin(), cs.deform.end());
-        arena.push_back(pad);
-        sd.deform_len = (uint32_t)cs.deform.size() + 1;
-      }
-      sd.K = cs.K;
-      sd.is_complex = cs.is_complex ? 1 : 0;
-      sd.sector_id = cs.sector_id;
-      sd.n_mem_main = cs.n_mem_main;
-      sd.n_mem_deform = cs.n_mem_deform;
-      sd.lambda = cs.lambda;
-      if (info) info[s] = cs.info;
-      pg->sec_host.push_back(sd);
-      pg->host.push_back(std::move(cs));
+    };
+    unsigned nthr = std::min<unsigned>(std::max(1u, std::thread::hardware_concurrency()), 32u);
+    nthr = std::min<unsigned>(nthr, (unsigned)((nsectors + 7) / 8));
+    if (nthr <= 1) {
+      worker();
+    } else {
+      std::vector<std::thread> pool;
+      for (unsigned t = 0; t < nthr; ++t) pool.emplace_back(worker);
+      for (auto &t : pool) t.join();
     }
-  } catch (fx::CompileError &e) {
-    delete pg;
-    return fail(ctx, e.code, e.msg);
+    if (err_sector < nsectors) {
+      delete pg;
+      return fail(ctx, err.code, err.msg);
+    }
+  }
+  for (int s = 0; s < nsectors; ++s) {
+    fx::CompiledSector &cs = compiled[s];
+    fx_sector_dev sd{};
+    fx_ins pad{};
+    pad.op = FX_END;
+    sd.main_off = (uint32_t)arena.size();
+    arena.insert(arena.end(), cs.main.begin(), cs.main.end());
+    arena.push_back(pad);
+    sd.main_len = (uint32_t)cs.main.size() + 1;
+    if (!cs.deform.empty()) {
+      sd.deform_off = (uint32_t)arena.size();
+      arena.insert(arena.end(), cs.deform.begin(), cs.deform.end());
+      arena.push_back(pad);
+      sd.deform_len = (uint32_t)cs.deform.size() + 1;
+    }
+    sd.K = cs.K;
+    sd.is_complex = cs.is_complex ? 1 : 0;
+    sd.sector_id = cs.sector_id;
+    sd.n_mem_main = cs.n_mem_main;
+    sd.n_mem_deform = cs.n_mem_deform;
+    sd.lambda = cs.lambda;
+    if (info) info[s] = cs.info;
+    pg->sec_host.push_back(sd);
+    pg->host.push_back(std::move(cs));
   }
   cudaSetDevice(ctx->device);
   pg->arena_len = arena.size();

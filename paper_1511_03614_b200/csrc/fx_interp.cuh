@@ -5,17 +5,18 @@
 // is warp-uniform (every thread of a block runs the same program), and every operand register
 // is named by the opcode, so the handlers are plain DFMA/DMUL/DADD on physical registers: no
 // indexed register file, no per-point temporaries in memory (contrast PAPER.md:126).
+//
+// Two levels:
+//   fast path  fx_fast<T,NX,P>::run  -- generated inline PTX (gen_interp_ptx.py): fetch, brx.idx
+//              dispatch and the arithmetic handlers, threaded code; runs until it meets an opcode
+//              it does not implement and hands that instruction back;
+//   slow path  the switch below, in C++: outputs (FX_OUT), FX_END and the rare library-backed
+//              operations (log, exp; complex division, square root).  A few per point.
 #ifndef FX_INTERP_CUH
 #define FX_INTERP_CUH
 
 #include "fx_isa.h"
 #include "fx_math.cuh"
-
-template <int r, typename T, int NX, int P>
-__device__ __forceinline__ T (&fx_reg(T (&X)[NX][P], T (&S)[FX_NS][P]))[P] {
-  if constexpr (r < FX_NXMAX) return X[r < NX ? r : 0];
-  else return S[r - FX_NXMAX];
-}
 
 template <typename T>
 struct fx_mem;  // shared-memory spill slots, one column per thread
@@ -41,41 +42,27 @@ struct fx_mem<cplx> {
 
 #define FX_PLOOP _Pragma("unroll") for (int p = 0; p < P; ++p)
 
-#define FX_REP8(M, ...) M(0, __VA_ARGS__) M(1, __VA_ARGS__) M(2, __VA_ARGS__) M(3, __VA_ARGS__) \
-  M(4, __VA_ARGS__) M(5, __VA_ARGS__) M(6, __VA_ARGS__) M(7, __VA_ARGS__)
-#define FX_REP20(M, ...) M(0, __VA_ARGS__) M(1, __VA_ARGS__) M(2, __VA_ARGS__) M(3, __VA_ARGS__) \
-  M(4, __VA_ARGS__) M(5, __VA_ARGS__) M(6, __VA_ARGS__) M(7, __VA_ARGS__) M(8, __VA_ARGS__) \
-  M(9, __VA_ARGS__) M(10, __VA_ARGS__) M(11, __VA_ARGS__) M(12, __VA_ARGS__) M(13, __VA_ARGS__) \
-  M(14, __VA_ARGS__) M(15, __VA_ARGS__) M(16, __VA_ARGS__) M(17, __VA_ARGS__) M(18, __VA_ARGS__) \
-  M(19, __VA_ARGS__)
+template <typename T, int NX, int P>
+struct fx_fast;  // specialised by the generated file for the variants FX_WANT selects
 
-// one handler of a register family: Rr names R[r] statically
-#define FX_CASE_R(r, base, stmt)                       \
-  case (base) + (r): {                                 \
-    if constexpr ((r) >= FX_NXMAX || (r) < NX) {       \
-      T(&Rr)[P] = fx_reg<(r), T, NX, P>(X, S);         \
-      FX_PLOOP { stmt; }                               \
-    }                                                  \
-    break;                                             \
-  }
-// A = A*R[r] + S[j]
-#define FX_CASE_RS_J(j, r)                                              \
-  case FX_FMA_AR_S + (r) * FX_NS + (j): {                               \
-    if constexpr ((r) >= FX_NXMAX || (r) < NX) {                        \
-      T(&Rr)[P] = fx_reg<(r), T, NX, P>(X, S);                          \
-      FX_PLOOP { A[p] = t_fma(A[p], Rr[p], S[j][p]); }                  \
-    }                                                                   \
-    break;                                                              \
-  }
-#define FX_CASE_RS(r, unused) FX_REP8(FX_CASE_RS_J, r)
-#define FX_CASE_ST(j, unused) \
-  case FX_ST_S + (j): {       \
-    FX_PLOOP { S[j][p] = A[p]; } \
-    break;                    \
-  }
+#ifndef FX_WANT
+#error "define FX_WANT(is_cplx, nx, p) before including fx_interp.cuh"
+#endif
+#include "fx_interp_gen.inc"
+
+// R[r] for a run-time r: only the slow path uses it (complex division by a register)
+template <typename T, int NX, int P>
+__device__ __forceinline__ void fx_reg_dyn(int r, const T (&X)[NX][P], const T (&S)[FX_NS][P], T (&out)[P]) {
+#pragma unroll
+  for (int k = 0; k < NX; ++k)
+    if (r == k) FX_PLOOP { out[p] = X[k][p]; }
+#pragma unroll
+  for (int j = 0; j < FX_NS; ++j)
+    if (r == FX_NXMAX + j) FX_PLOOP { out[p] = S[j][p]; }
+}
 
 // Walk `prog` (shared memory) for the P points whose variables are in X.  `sink(k, A)` receives
-// output k (FX_OUT).  M are this thread's spill slots.
+// output k (FX_OUT).  M are this thread's spill slots (stride must be FX_THREADS).
 template <typename T, int NX, int P, class Sink>
 __device__ __forceinline__ void fx_run(const fx_ins *prog, T (&X)[NX][P], const fx_mem<T> M, Sink &sink) {
   T A[P];
@@ -83,52 +70,40 @@ __device__ __forceinline__ void fx_run(const fx_ins *prog, T (&X)[NX][P], const 
   FX_PLOOP { A[p] = t_from_real(0.0, T{}); }
 #pragma unroll
   for (int j = 0; j < FX_NS; ++j) FX_PLOOP { S[j][p] = t_from_real(0.0, T{}); }
-  const uint4 *pc = reinterpret_cast<const uint4 *>(prog);
-  uint4 w = *pc;
+  uint32_t pc = (uint32_t)__cvta_generic_to_shared(prog);
+  const uint32_t mem = (uint32_t)__cvta_generic_to_shared(M.base);
   for (;;) {
-    const uint4 cur = w;
-    ++pc;
-    w = *pc;  // prefetch the next instruction (programs end with FX_END followed by padding)
-    const int op = cur.x & 0xffff;
-    const int aux = cur.x >> 16;
-    const double imm = __hiloint2double((int)cur.w, (int)cur.z);
-    switch (op) {
-      FX_REP20(FX_CASE_R, FX_FMA_AR_C, A[p] = t_fma_c(A[p], Rr[p], imm))
-      FX_REP20(FX_CASE_R, FX_FMA_RC_A, A[p] = t_fma_rc(Rr[p], imm, A[p]))
-      FX_REP20(FX_CASE_R, FX_MUL_R, A[p] = t_mul(A[p], Rr[p]))
-      FX_REP20(FX_CASE_R, FX_ADD_R, A[p] = t_add(A[p], Rr[p]))
-      FX_REP20(FX_CASE_R, FX_SUB_R, A[p] = t_sub(A[p], Rr[p]))
-      FX_REP20(FX_CASE_R, FX_RSUB_R, A[p] = t_sub(Rr[p], A[p]))
-      FX_REP20(FX_CASE_R, FX_LD_R, A[p] = Rr[p])
-      FX_REP20(FX_CASE_R, FX_MULC_R, A[p] = t_mulc(Rr[p], imm))
-      FX_REP20(FX_CASE_R, FX_DIV_R, A[p] = t_div(A[p], Rr[p]))
-      FX_REP20(FX_CASE_R, FX_RDIV_R, A[p] = t_div(Rr[p], A[p]))
-      FX_REP20(FX_CASE_R, FX_FMA_AR_M, A[p] = t_fma(A[p], Rr[p], M.ld(aux, p, P)))
-      FX_REP20(FX_CASE_RS, 0)
-      FX_REP8(FX_CASE_ST, 0)
-      case FX_LDC: FX_PLOOP { A[p] = t_from_real(imm, T{}); } break;
-      case FX_ADDC: FX_PLOOP { A[p] = t_addc(A[p], imm); } break;
-      case FX_MULC: FX_PLOOP { A[p] = t_mulc(A[p], imm); } break;
-      case FX_RSUBC: FX_PLOOP { A[p] = t_rsubc(imm, A[p]); } break;
-      case FX_DIVC: FX_PLOOP { A[p] = t_divc(A[p], imm); } break;
-      case FX_RDIVC: FX_PLOOP { A[p] = t_rdivc(imm, A[p]); } break;
-      case FX_LDM: FX_PLOOP { A[p] = M.ld(aux, p, P); } break;
-      case FX_STM: FX_PLOOP { M.st(aux, p, P, A[p]); } break;
-      case FX_ADDM: FX_PLOOP { A[p] = t_add(A[p], M.ld(aux, p, P)); } break;
-      case FX_SUBM: FX_PLOOP { A[p] = t_sub(A[p], M.ld(aux, p, P)); } break;
-      case FX_RSUBM: FX_PLOOP { A[p] = t_sub(M.ld(aux, p, P), A[p]); } break;
-      case FX_MULM: FX_PLOOP { A[p] = t_mul(A[p], M.ld(aux, p, P)); } break;
-      case FX_DIVM: FX_PLOOP { A[p] = t_div(A[p], M.ld(aux, p, P)); } break;
-      case FX_RDIVM: FX_PLOOP { A[p] = t_div(M.ld(aux, p, P), A[p]); } break;
-      case FX_FMA_AM_C: FX_PLOOP { A[p] = t_fma_c(A[p], M.ld(aux, p, P), imm); } break;
-      case FX_FMA_MC_A: FX_PLOOP { A[p] = t_fma_rc(M.ld(aux, p, P), imm, A[p]); } break;
-      case FX_NEG: FX_PLOOP { A[p] = t_neg(A[p]); } break;
-      case FX_SQR: FX_PLOOP { A[p] = t_mul(A[p], A[p]); } break;
-      case FX_LOG: FX_PLOOP { A[p] = t_log(A[p]); } break;
-      case FX_EXP: FX_PLOOP { A[p] = t_exp(A[p]); } break;
-      case FX_SQRT: FX_PLOOP { A[p] = t_sqrt(A[p]); } break;
-      case FX_OUT: sink(aux, A); break;
-      default: return;  // FX_END
+    uint32_t w0, w2, w3;
+    fx_fast<T, NX, P>::run(A, X, S, pc, mem, w0, w2, w3);
+    const int op = w0 & 0xffff;
+    const int aux = w0 >> 16;
+    const double imm = __hiloint2double((int)w3, (int)w2);
+    if (op == FX_OUT) {
+      sink(aux, A);
+    } else if (op == FX_LOG) {
+      FX_PLOOP { A[p] = t_log(A[p]); }
+    } else if (op == FX_EXP) {
+      FX_PLOOP { A[p] = t_exp(A[p]); }
+    } else if (op == FX_SQRT) {
+      FX_PLOOP { A[p] = t_sqrt(A[p]); }
+    } else if (op == FX_RDIVC) {
+      FX_PLOOP { A[p] = t_rdivc(imm, A[p]); }
+    } else if (op == FX_DIVM) {
+      FX_PLOOP { A[p] = t_div(A[p], M.ld(aux, p, P)); }
+    } else if (op == FX_RDIVM) {
+      FX_PLOOP { A[p] = t_div(M.ld(aux, p, P), A[p]); }
+    } else if (op >= FX_DIV_R && op < FX_DIV_R + FX_NR) {
+      T R[P];
+      FX_PLOOP { R[p] = A[p]; }
+      fx_reg_dyn<T, NX, P>(op - FX_DIV_R, X, S, R);
+      FX_PLOOP { A[p] = t_div(A[p], R[p]); }
+    } else if (op >= FX_RDIV_R && op < FX_RDIV_R + FX_NR) {
+      T R[P];
+      FX_PLOOP { R[p] = A[p]; }
+      fx_reg_dyn<T, NX, P>(op - FX_RDIV_R, X, S, R);
+      FX_PLOOP { A[p] = t_div(R[p], A[p]); }
+    } else {
+      return;  // FX_END (or an opcode naming a variable this kernel does not have)
     }
   }
 }

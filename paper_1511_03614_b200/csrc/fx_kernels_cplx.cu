@@ -6,11 +6,11 @@
 //     o_k(z) * det J                                      complex program, LU with partial pivoting
 // Compiled once per dimension N (-DFX_N=1..8) so the N x N elimination is fully unrolled on
 // registers.  SURVEY 8(a) steps A4, A5 (complex), A6, A7.
-#include "fx_device_common.cuh"
-
 #ifndef FX_N
 #error "compile with -DFX_N=<dimension 1..8>"
 #endif
+#define FX_WANT(is_cplx, nx, p) ((nx) == FX_N && (p) == 2)  // real (deformation program) and complex, P = 2
+#include "fx_device_common.cuh"
 
 namespace {
 

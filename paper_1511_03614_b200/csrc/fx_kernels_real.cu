@@ -2,6 +2,7 @@
 // points made on the device, program walk, accumulation of sum g and sum g^2 per order
 // (SURVEY 8(a) A1-A3, A5-A7, A8 histogram part).  Replaces the reference's CUDA kernel of
 // PAPER.md:118-126 (thread per point, temporaries in GPU memory, points uploaded per batch).
+#define FX_WANT(is_cplx, nx, p) ((is_cplx) == 0 && (p) == 4)  // fast-path variants this file instantiates
 #include "fx_device_common.cuh"
 
 namespace {

@@ -1,0 +1,288 @@
+#!/usr/bin/env python
+"""Generates fx_interp_gen.inc: the fast path of the program walk as inline PTX.
+
+Why PTX: nvcc lowers a C++ `switch` over ~400 opcodes to a compare-and-branch tree, and ptxas
+then re-copies the whole per-thread register state (X, S, A: 140+ registers) on every trip
+round the loop -- measured at ~600 cycles per interpreted op (profiles/r01_switch_baseline.md).
+Here the dispatch is one `brx.idx` through a `.branchtargets` table (SASS: BRX), every handler
+names its operand registers statically and ends with its own fetch + dispatch (threaded code),
+so the loop is: LDS.128 (fetch), LOP (decode), BRX, P x DFMA.
+
+One function per (arithmetic type, NX variables, P points per thread):
+
+    fx_fast_<real|cplx>_<NX>_<P>(A, X, S, pc, mem, w0, w2, w3)
+
+walks instructions from shared-memory byte address `pc` until it meets an opcode it does not
+handle (FX_OUT, FX_END, log/exp, complex division ...), and returns that instruction's words in
+(w0, w2, w3) with pc pointing past it; the C++ caller (fx_interp.cuh) handles it and re-enters.
+
+    python gen_interp_ptx.py > fx_interp_gen.inc      (build.py does this)
+
+The opcode numbers are parsed from fx_isa.h, so the two cannot drift apart.
+"""
+import os
+import re
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+# threaded code (every handler ends with its own fetch + brx.idx) saves one BRA per op, but gives
+# ptxas a control-flow graph of (#handlers x #opcodes) edges: its compile time explodes (> 30 min
+# for NX = 8).  With one shared dispatch point the graph has #handlers + #opcodes edges.
+THREADED = False
+THREADS = 128   # FX_THREADS: stride (in doubles) between spill slots of one thread
+NXMAX, NS = 12, 8
+
+
+def parse_isa():
+    txt = open(os.path.join(HERE, "fx_isa.h")).read()
+    body = txt[txt.index("enum fx_op"):]
+    body = body[body.index("{") + 1:body.index("};")]
+    ops, val = {}, 0
+    for line in body.splitlines():
+        line = line.split("//")[0].strip().rstrip(",")
+        if not line:
+            continue
+        m = re.match(r"(\w+)\s*=\s*(\d+)$", line)
+        if m:
+            val = int(m.group(2))
+            ops[m.group(1)] = val
+        else:
+            ops[line] = val
+        val += 1
+    return ops
+
+
+OPS = parse_isa()
+NOPS = OPS["FX_NOPS"]
+
+
+class Gen:
+    def __init__(self, cplx, nx, p):
+        self.cplx, self.nx, self.p = cplx, nx, p
+        self.operands = []       # (constraint, c-expression)
+        self.lines = []
+        self.C = 2 if cplx else 1
+
+    # ---- operands ---------------------------------------------------------------------
+    def opnd(self, constraint, expr):
+        self.operands.append((constraint, expr))
+        return "%%%d" % (len(self.operands) - 1)
+
+    def setup(self):
+        comp = (".re", ".im") if self.cplx else ("",)
+        self.A = [[self.opnd("+d", f"A[{p}]{c}") for c in comp] for p in range(self.p)]
+        self.X = [[[self.opnd("+d", f"X[{k}][{p}]{c}") for c in comp] for p in range(self.p)] for k in range(self.nx)]
+        self.S = [[[self.opnd("+d", f"S[{j}][{p}]{c}") for c in comp] for p in range(self.p)] for j in range(NS)]
+        self.pc = self.opnd("+r", "pc")
+        self.w0 = self.opnd("=r", "w0")
+        self.w2 = self.opnd("=r", "w2")
+        self.w3 = self.opnd("=r", "w3")
+        self.mem = self.opnd("r", "mem")
+
+    def R(self, r):
+        return self.X[r] if r < NXMAX else self.S[r - NXMAX]
+
+    def emit(self, s):
+        self.lines.append(s)
+
+    def dispatch(self):
+        self.emit(f"ld.shared.v4.u32 {{{self.w0},w1,{self.w2},{self.w3}}}, [{self.pc}];")
+        self.emit(f"add.u32 {self.pc}, {self.pc}, 16;")
+        self.emit(f"and.b32 op, {self.w0}, 0xffff;")
+        self.emit(f"mov.b64 imm, {{{self.w2},{self.w3}}};")
+        self.emit("brx.idx op, TBL;")
+
+    # ---- memory slots -----------------------------------------------------------------
+    def mem_addr(self):
+        """ma = mem + aux * (C*P*THREADS*8)"""
+        self.emit(f"shr.u32 ma, {self.w0}, 16;")
+        self.emit(f"mad.lo.u32 ma, ma, {self.C * self.p * THREADS * 8}, {self.mem};")
+
+    def mem_off(self, p, c):
+        return (c * self.p + p) * THREADS * 8
+
+    def ld_mem(self, p):
+        """loads slot value of point p into m0 (re) [, m1 (im)]"""
+        for c in range(self.C):
+            self.emit(f"ld.shared.f64 m{c}, [ma+{self.mem_off(p, c)}];")
+        return ["m0", "m1"][:self.C]
+
+    # ---- arithmetic templates; a, b, c are component lists; result assigned to a ------
+    def fma_full(self, a, b, c):          # a = a*b + c
+        if not self.cplx:
+            self.emit(f"fma.rn.f64 {a[0]}, {a[0]}, {b[0]}, {c[0]};")
+            return
+        self.emit(f"neg.f64 t0, {a[1]};")
+        self.emit(f"fma.rn.f64 t0, t0, {b[1]}, {c[0]};")
+        self.emit(f"fma.rn.f64 t1, {a[1]}, {b[0]}, {c[1]};")
+        self.emit(f"fma.rn.f64 t1, {a[0]}, {b[1]}, t1;")
+        self.emit(f"fma.rn.f64 {a[0]}, {a[0]}, {b[0]}, t0;")
+        self.emit(f"mov.f64 {a[1]}, t1;")
+
+    def fma_c(self, a, b, imm="imm"):     # a = a*b + imm (imm real)
+        if not self.cplx:
+            self.emit(f"fma.rn.f64 {a[0]}, {a[0]}, {b[0]}, {imm};")
+            return
+        self.emit(f"neg.f64 t0, {a[1]};")
+        self.emit(f"fma.rn.f64 t0, t0, {b[1]}, {imm};")
+        self.emit(f"mul.rn.f64 t1, {a[1]}, {b[0]};")
+        self.emit(f"fma.rn.f64 t1, {a[0]}, {b[1]}, t1;")
+        self.emit(f"fma.rn.f64 {a[0]}, {a[0]}, {b[0]}, t0;")
+        self.emit(f"mov.f64 {a[1]}, t1;")
+
+    def fma_rc(self, a, r, imm="imm"):    # a = r*imm + a
+        for c in range(self.C):
+            self.emit(f"fma.rn.f64 {a[c]}, {r[c]}, {imm}, {a[c]};")
+
+    def mul(self, a, b):                  # a = a*b
+        if not self.cplx:
+            self.emit(f"mul.rn.f64 {a[0]}, {a[0]}, {b[0]};")
+            return
+        self.emit(f"mul.rn.f64 t0, {a[1]}, {b[1]};")
+        self.emit("neg.f64 t0, t0;")
+        self.emit(f"mul.rn.f64 t1, {a[1]}, {b[0]};")
+        self.emit(f"fma.rn.f64 t1, {a[0]}, {b[1]}, t1;")
+        self.emit(f"fma.rn.f64 {a[0]}, {a[0]}, {b[0]}, t0;")
+        self.emit(f"mov.f64 {a[1]}, t1;")
+
+    def comp2(self, ins, a, x, y):        # a = x <ins> y componentwise
+        for c in range(self.C):
+            self.emit(f"{ins} {a[c]}, {x[c]}, {y[c]};")
+
+    # ---- handlers ---------------------------------------------------------------------
+    def handler(self, label, body_per_point, pre=None):
+        self.emit(f"{label}:")
+        if pre:
+            pre()
+        for p in range(self.p):
+            body_per_point(p)
+        if THREADED:
+            self.dispatch()
+        else:
+            self.emit("bra.uni NEXT;")
+
+    def build(self):
+        self.setup()
+        table = ["EXIT"] * NOPS
+        A, cx = self.A, self.cplx
+
+        def reg_family(base, name, body, ok=True):
+            for r in range(NXMAX + NS):
+                if not ok or (r < NXMAX and r >= self.nx):
+                    continue
+                lab = f"H_{name}_{r}"
+                table[OPS[base] + r] = lab
+                self.handler(lab, lambda p, r=r: body(A[p], self.R(r)[p], p), pre=self.mem_addr if name == "FMA_AR_M" else None)
+
+        reg_family("FX_FMA_AR_C", "FMA_AR_C", lambda a, r, p: self.fma_c(a, r))
+        reg_family("FX_FMA_RC_A", "FMA_RC_A", lambda a, r, p: self.fma_rc(a, r))
+        reg_family("FX_MUL_R", "MUL_R", lambda a, r, p: self.mul(a, r))
+        reg_family("FX_ADD_R", "ADD_R", lambda a, r, p: self.comp2("add.rn.f64", a, a, r))
+        reg_family("FX_SUB_R", "SUB_R", lambda a, r, p: self.comp2("sub.rn.f64", a, a, r))
+        reg_family("FX_RSUB_R", "RSUB_R", lambda a, r, p: self.comp2("sub.rn.f64", a, r, a))
+        reg_family("FX_LD_R", "LD_R", lambda a, r, p: [self.emit(f"mov.f64 {a[c]}, {r[c]};") for c in range(self.C)])
+        reg_family("FX_MULC_R", "MULC_R", lambda a, r, p: [self.emit(f"mul.rn.f64 {a[c]}, {r[c]}, imm;") for c in range(self.C)])
+        reg_family("FX_DIV_R", "DIV_R", lambda a, r, p: self.emit(f"div.rn.f64 {a[0]}, {a[0]}, {r[0]};"), ok=not cx)
+        reg_family("FX_RDIV_R", "RDIV_R", lambda a, r, p: self.emit(f"div.rn.f64 {a[0]}, {r[0]}, {a[0]};"), ok=not cx)
+        reg_family("FX_FMA_AR_M", "FMA_AR_M", lambda a, r, p: self.fma_full(a, r, self.ld_mem(p)))
+        for r in range(NXMAX + NS):
+            if r < NXMAX and r >= self.nx:
+                continue
+            for j in range(NS):
+                lab = f"H_FMA_AR_S_{r}_{j}"
+                table[OPS["FX_FMA_AR_S"] + r * NS + j] = lab
+                self.handler(lab, lambda p, r=r, j=j: self.fma_full(A[p], self.R(r)[p], self.S[j][p]))
+        for j in range(NS):
+            lab = f"H_ST_S_{j}"
+            table[OPS["FX_ST_S"] + j] = lab
+            self.handler(lab, lambda p, j=j: [self.emit(f"mov.f64 {self.S[j][p][c]}, {A[p][c]};") for c in range(self.C)])
+
+        def single(name, body, pre=None, ok=True):
+            if not ok:
+                return
+            lab = "H_" + name
+            table[OPS["FX_" + name]] = lab
+            self.handler(lab, body, pre)
+
+        def ldc(p):
+            self.emit(f"mov.f64 {A[p][0]}, imm;")
+            if cx:
+                self.emit(f"mov.f64 {A[p][1]}, zero;")
+
+        def rsubc(p):
+            self.emit(f"sub.rn.f64 {A[p][0]}, imm, {A[p][0]};")
+            if cx:
+                self.emit(f"neg.f64 {A[p][1]}, {A[p][1]};")
+
+        single("LDC", ldc)
+        single("ADDC", lambda p: self.emit(f"add.rn.f64 {A[p][0]}, {A[p][0]}, imm;"))
+        single("MULC", lambda p: [self.emit(f"mul.rn.f64 {A[p][c]}, {A[p][c]}, imm;") for c in range(self.C)])
+        single("RSUBC", rsubc)
+        single("DIVC", lambda p: [self.emit(f"div.rn.f64 {A[p][c]}, {A[p][c]}, imm;") for c in range(self.C)])
+        single("RDIVC", lambda p: self.emit(f"div.rn.f64 {A[p][0]}, imm, {A[p][0]};"), ok=not cx)
+        single("LDM", lambda p: [self.emit(f"mov.f64 {A[p][c]}, {m};") for c, m in enumerate(self.ld_mem(p))], self.mem_addr)
+        single("STM", lambda p: [self.emit(f"st.shared.f64 [ma+{self.mem_off(p, c)}], {A[p][c]};") for c in range(self.C)],
+               self.mem_addr)
+        single("ADDM", lambda p: self.comp2("add.rn.f64", A[p], A[p], self.ld_mem(p)), self.mem_addr)
+        single("SUBM", lambda p: self.comp2("sub.rn.f64", A[p], A[p], self.ld_mem(p)), self.mem_addr)
+        single("RSUBM", lambda p: self.comp2("sub.rn.f64", A[p], self.ld_mem(p), A[p]), self.mem_addr)
+        single("MULM", lambda p: self.mul(A[p], self.ld_mem(p)), self.mem_addr)
+        single("DIVM", lambda p: self.emit(f"div.rn.f64 {A[p][0]}, {A[p][0]}, {self.ld_mem(p)[0]};"), self.mem_addr, ok=not cx)
+        single("RDIVM", lambda p: self.emit(f"div.rn.f64 {A[p][0]}, {self.ld_mem(p)[0]}, {A[p][0]};"), self.mem_addr, ok=not cx)
+        single("FMA_AM_C", lambda p: self.fma_c(A[p], self.ld_mem(p)), self.mem_addr)
+        single("FMA_MC_A", lambda p: self.fma_rc(A[p], self.ld_mem(p)), self.mem_addr)
+        single("NEG", lambda p: [self.emit(f"neg.f64 {A[p][c]}, {A[p][c]};") for c in range(self.C)])
+        single("SQR", lambda p: self.mul(A[p], A[p]))
+        single("SQRT", lambda p: self.emit(f"sqrt.rn.f64 {A[p][0]}, {A[p][0]};"), ok=not cx)
+        return table
+
+    def function(self):
+        table = self.build()
+        handlers = self.lines
+        self.lines = []
+        kind = "cplx" if self.cplx else "real"
+        T = "cplx" if self.cplx else "double"
+        name = f"fx_fast_{kind}_{self.nx}_{self.p}"
+        out = [f"#if FX_WANT({int(self.cplx)}, {self.nx}, {self.p})",
+               f"__device__ __forceinline__ void {name}({T} (&A)[{self.p}], {T} (&X)[{self.nx}][{self.p}], "
+               f"{T} (&S)[{NS}][{self.p}], uint32_t &pc, uint32_t mem, uint32_t &w0, uint32_t &w2, uint32_t &w3) {{",
+               "  asm volatile(", '    "{\\n"',
+               '    ".reg .u32 w1, op, ma;\\n"', '    ".reg .f64 imm, zero, t0, t1, m0, m1;\\n"',
+               '    "mov.f64 zero, 0d0000000000000000;\\n"']
+        tl = ", ".join(table)
+        out.append(f'    "TBL: .branchtargets {tl};\\n"')
+        self.emit("NEXT:")
+        self.dispatch()
+        for ln in self.lines + handlers:
+            out.append(f'    "{ln}\\n"')
+        out.append('    "EXIT:\\n"')
+        out.append('    "}\\n"')
+        outs = [o for o in self.operands if o[0][0] in "+="]
+        ins = [o for o in self.operands if o[0][0] not in "+="]
+        # outputs must be numbered first: check the numbering matches the order used above
+        order = outs + ins
+        assert order == self.operands, "operand order must be outputs then inputs"
+        out.append("    : " + ", ".join(f'"{c}"({e})' for c, e in outs))
+        out.append("    : " + ", ".join(f'"{c}"({e})' for c, e in ins))
+        out.append('    : "memory");')
+        out.append("}")
+        out.append(f"template <> struct fx_fast<{T}, {self.nx}, {self.p}> {{")
+        out.append(f"  static __device__ __forceinline__ void run({T} (&A)[{self.p}], {T} (&X)[{self.nx}][{self.p}], "
+                   f"{T} (&S)[{NS}][{self.p}], uint32_t &pc, uint32_t mem, uint32_t &w0, uint32_t &w2, uint32_t &w3) {{")
+        out.append(f"    {name}(A, X, S, pc, mem, w0, w2, w3);")
+        out.append("  }")
+        out.append("};")
+        out.append("#endif")
+        return "\n".join(out)
+
+
+def main():
+    variants = [(False, nx, 4) for nx in (4, 8, 12)] + [(False, nx, 2) for nx in range(1, 9)] + \
+               [(True, nx, 2) for nx in range(1, 9)]
+    print("// GENERATED by gen_interp_ptx.py -- do not edit.  See that file for the design.")
+    for cplx, nx, p in variants:
+        print(Gen(cplx, nx, p).function())
+
+
+if __name__ == "__main__":
+    main()

@@ -79,9 +79,11 @@ def test_periodising_transform(fb, ctx, r):
     x, xbar, w = ctx.transform_points(rule, t)
     xo, xbo, wo = OP.korobov_transform(OP.unit_from_t(t), r)
     wo = np.prod(wo, axis=1)
-    # x and 1-x each carry full relative accuracy at both faces (R4)
-    assert np.max(np.abs(x - xo.astype(float)) / xo.astype(float)) < 4e-15
-    assert np.max(np.abs(xbar - xbo.astype(float)) / xbo.astype(float)) < 4e-15
+    # x and 1-x each carry full relative accuracy at both faces (R4).  The alternating sum of
+    # phi_r at v -> 1/2 has condition number ~12 (r=3) .. ~240 (r=6): DESIGN.md "Tolerances".
+    tol = 4e-15 if r <= 4 else 4e-14
+    assert np.max(np.abs(x - xo.astype(float)) / xo.astype(float)) < tol
+    assert np.max(np.abs(xbar - xbo.astype(float)) / xbo.astype(float)) < tol
     ok = wo.astype(float) > 1e-290          # u = 2^-53 underflows FP64 for r >= 5
     assert np.max(np.abs(w[ok] - wo[ok].astype(float)) / wo[ok].astype(float)) < 2e-14
 
@@ -101,9 +103,10 @@ def _eval_case(ctx, wl, nsec, npts, seed):
     rng = np.random.default_rng(seed)
     x = rng.random((npts, wl.dim))
     # points near the faces of the cube, where the integrands vary fastest
-    x[: wl.dim] = 0.5
-    for k in range(wl.dim):
-        x[k, k] = 1e-9
+    if npts > wl.dim:
+        x[: wl.dim] = 0.5
+        for k in range(wl.dim):
+            x[k, k] = 1e-9
     worst = 0.0
     for si in range(nsec):
         got = ctx.eval_points(prog, si, x)
@@ -442,7 +445,7 @@ def test_nonfinite_is_reported(fb, ctx):
 
 
 @pytest.mark.parametrize("text,dim,code", [
-    ("1;\n0;\nx[1]+;\n|", 1, -1), ("1;\n0;\nx[1]+0.2;\n", 1, -1), ("1;\n0;\nq[1];\n|", 1, -1),
+    ("1;\n0;\nx[1]+;\n|", 1, -1), ("1;\n0;\nx[1]+0.2;\n| 7", 1, -1), ("1;\n0;\nq[1];\n|", 1, -1),
     ("1;\n0;\nx[2];\n|", 1, -2), ("1;\n1;\nx[1];\nf[2];\n|", 1, -1), ("1;\n0;\nPolyGamma[9,9];\n|", 1, -1),
     ("1;\n0;\np[x[1],x[1]];\n|", 1, -1), ("13;\n0;\nx[1];\n|", 13, -2)])
 def test_compile_errors(fb, ctx, text, dim, code):

@@ -128,16 +128,29 @@ def _mono_ops(exps) -> int:
     return max(nz - 1, 0) + sum(1 for e in exps if e > 1)
 
 
+_TERM_CACHE = {}
+
+
+def _term_text(c, e):
+    """Text and operator-node count of one term c * monomial (memoised: the C3 size loop re-renders)."""
+    key = (c, e)
+    hit = _TERM_CACHE.get(key)
+    if hit is None:
+        if len(_TERM_CACHE) > 200000:
+            _TERM_CACHE.clear()
+        mt = _mono_text(e)
+        hit = (f"{_num(c)}*{mt}", 1 + _mono_ops(e)) if mt else (_num(c), 0)
+        _TERM_CACHE[key] = hit
+    return hit
+
+
 def _poly_text(mons):
     """Text and operator-node count of sum_m c_m * monomial_m."""
     terms, ops = [], 0
     for c, e in mons:
-        mt = _mono_text(e)
-        if mt:
-            terms.append(f"{_num(c)}*{mt}")
-            ops += 1 + _mono_ops(e)
-        else:
-            terms.append(_num(c))
+        t, o = _term_text(c, e)
+        terms.append(t)
+        ops += o
     ops += len(terms) - 1
     return "+".join(terms), ops
 
