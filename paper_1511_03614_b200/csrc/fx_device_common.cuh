@@ -40,8 +40,42 @@ __device__ __forceinline__ void fx_copy_program(fx_ins *dst, const fx_ins *src, 
   for (int i = threadIdx.x; i < n; i += blockDim.x) d[i] = s[i];
 }
 
+// Out-of-line helpers: the evaluation kernels call them once per coordinate.  Keeping one copy of
+// each (instead of NX*P inlined copies) keeps the per-batch code outside the program walk small, so
+// it does not evict the walk's handlers from the 32 KB instruction cache (profiles/r01_*.md).
+struct fx_coord {
+  double x, xbar, w;
+};
+struct fx_tpair {
+  uint64_t e, o;
+};
+
+static __device__ __noinline__ fx_coord fx_lattice_coord(uint64_t t, const fx_transform *tf) {
+  fx_coord c;
+  korobov_transform(*tf, unit_from_t(t), c.x, c.xbar, c.w);
+  return c;
+}
+
+static __device__ __noinline__ fx_tpair fx_philox_pair(uint64_t seed, uint32_t sector_id, uint32_t tag, uint32_t it, uint64_t j,
+                                                uint32_t kb) {
+  fx_tpair r;
+  philox_t_pair(seed, sector_id, tag, it, j, kb, r.e, r.o);
+  return r;
+}
+
+struct fx_vcoord {
+  double x, w;
+  int bin;
+};
+static __device__ __noinline__ fx_vcoord fx_vegas_coord(uint64_t t, int nbins, const double *edges) {
+  fx_vcoord c;
+  vegas_map_coord(t, nbins, edges, c.x, c.w, c.bin);
+  return c;
+}
+
 // Points j0..j0+P-1 of (sector, shift r / iteration) -> real x, xbar = 1-x, weight W, Vegas bins.
-template <int NX, int P>
+// RULE is a compile-time constant: each rule has its own kernel instantiation.
+template <int RULE, int NX, int P>
 __device__ __forceinline__ void fx_make_points(const fx_integrate_params &prm, int dim, uint32_t sector_id,
                                                const uint64_t *sh_delta, const double *sh_grid, uint64_t j0,
                                                uint64_t jend, double (&x)[NX][P], double (&xbar)[NX][P],
@@ -53,15 +87,18 @@ __device__ __forceinline__ void fx_make_points(const fx_integrate_params &prm, i
   }
 #pragma unroll
   for (int q = 0; q < (NX + 3) / 4; ++q) FX_PLOOP { bins[q][p] = 0; }
-  if (prm.rule == FIESTA_RULE_LATTICE) {
+  if constexpr (RULE == FIESTA_RULE_LATTICE) {
+    const fx_transform *tf = reinterpret_cast<const fx_transform *>(&prm.tf);
 #pragma unroll
     for (int k = 0; k < NX; ++k) {
       if (k < dim) {
+        // t_j = ((j g) mod 2^m) << (64-m) + Delta = j * (g << (64-m)) + Delta  (mod 2^64)
+        const uint64_t G = prm.log2_n ? (prm.genvec[k] << (64 - prm.log2_n)) : 0ull;
         FX_PLOOP {
-          uint64_t t = lattice_t(j0 + p, prm.genvec[k], prm.log2_n, sh_delta[k]);
-          double w;
-          korobov_transform(reinterpret_cast<const fx_transform &>(prm.tf), unit_from_t(t), x[k][p], xbar[k][p], w);
-          W[p] *= w;
+          const fx_coord c = fx_lattice_coord((j0 + p) * G + sh_delta[k], tf);
+          x[k][p] = c.x;
+          xbar[k][p] = c.xbar;
+          W[p] *= c.w;
         }
       } else {
         FX_PLOOP {
@@ -74,23 +111,22 @@ __device__ __forceinline__ void fx_make_points(const fx_integrate_params &prm, i
 #pragma unroll
     for (int kb = 0; kb < (NX + 1) / 2; ++kb) {
       FX_PLOOP {
-        uint64_t te = 0, to = 0;
-        if (2 * kb < dim) philox_t_pair(prm.seed, sector_id, FX_TAG_MC, (uint32_t)prm.iteration, j0 + p, kb, te, to);
+        fx_tpair tp{0ull, 0ull};
+        if (2 * kb < dim) tp = fx_philox_pair(prm.seed, sector_id, FX_TAG_MC, (uint32_t)prm.iteration, j0 + p, kb);
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
           const int k = 2 * kb + h;
           if (k < NX) {
-            uint64_t t = h ? to : te;
+            const uint64_t t = h ? tp.o : tp.e;
             if (k < dim) {
-              if (prm.rule == FIESTA_RULE_VEGAS) {
-                double wf;
-                int b;
-                vegas_map_coord(t, prm.nbins, sh_grid + k * (prm.nbins + 1), x[k][p], wf, b);
-                xbar[k][p] = 1.0 - x[k][p];
-                W[p] *= wf;
-                bins[k / 4][p] |= (uint32_t)b << (8 * (k % 4));
+              if constexpr (RULE == FIESTA_RULE_VEGAS) {
+                const fx_vcoord c = fx_vegas_coord(t, prm.nbins, sh_grid + k * (prm.nbins + 1));
+                x[k][p] = c.x;
+                xbar[k][p] = 1.0 - c.x;
+                W[p] *= c.w;
+                bins[k / 4][p] |= (uint32_t)c.bin << (8 * (k % 4));
               } else {
-                double u = unit_from_t(t);
+                const double u = unit_from_t(t);
                 x[k][p] = u;
                 xbar[k][p] = 1.0 - u;
               }

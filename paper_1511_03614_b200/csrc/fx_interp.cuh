@@ -50,6 +50,17 @@ struct fx_fast;  // specialised by the generated file for the variants FX_WANT s
 #endif
 #include "fx_interp_gen.inc"
 
+// Library-backed operations, out of line: one copy each instead of P inlined copies per call site
+// (instruction-cache footprint, see fx_device_common.cuh).
+static __device__ __noinline__ double fx_slow_log(double a) { return t_log(a); }
+static __device__ __noinline__ double fx_slow_exp(double a) { return t_exp(a); }
+static __device__ __noinline__ cplx fx_slow_log(cplx a) { return t_log(a); }
+static __device__ __noinline__ cplx fx_slow_exp(cplx a) { return t_exp(a); }
+static __device__ __noinline__ cplx fx_slow_sqrt(cplx a) { return t_sqrt(a); }
+__device__ __forceinline__ double fx_slow_sqrt(double a) { return t_sqrt(a); }
+static __device__ __noinline__ cplx fx_slow_div(cplx a, cplx b) { return t_div(a, b); }
+__device__ __forceinline__ double fx_slow_div(double a, double b) { return t_div(a, b); }
+
 // R[r] for a run-time r: only the slow path uses it (complex division by a register)
 template <typename T, int NX, int P>
 __device__ __forceinline__ void fx_reg_dyn(int r, const T (&X)[NX][P], const T (&S)[FX_NS][P], T (&out)[P]) {
@@ -81,27 +92,27 @@ __device__ __forceinline__ void fx_run(const fx_ins *prog, T (&X)[NX][P], const 
     if (op == FX_OUT) {
       sink(aux, A);
     } else if (op == FX_LOG) {
-      FX_PLOOP { A[p] = t_log(A[p]); }
+      FX_PLOOP { A[p] = fx_slow_log(A[p]); }
     } else if (op == FX_EXP) {
-      FX_PLOOP { A[p] = t_exp(A[p]); }
+      FX_PLOOP { A[p] = fx_slow_exp(A[p]); }
     } else if (op == FX_SQRT) {
-      FX_PLOOP { A[p] = t_sqrt(A[p]); }
+      FX_PLOOP { A[p] = fx_slow_sqrt(A[p]); }
     } else if (op == FX_RDIVC) {
       FX_PLOOP { A[p] = t_rdivc(imm, A[p]); }
     } else if (op == FX_DIVM) {
-      FX_PLOOP { A[p] = t_div(A[p], M.ld(aux, p, P)); }
+      FX_PLOOP { A[p] = fx_slow_div(A[p], M.ld(aux, p, P)); }
     } else if (op == FX_RDIVM) {
-      FX_PLOOP { A[p] = t_div(M.ld(aux, p, P), A[p]); }
+      FX_PLOOP { A[p] = fx_slow_div(M.ld(aux, p, P), A[p]); }
     } else if (op >= FX_DIV_R && op < FX_DIV_R + FX_NR) {
       T R[P];
       FX_PLOOP { R[p] = A[p]; }
       fx_reg_dyn<T, NX, P>(op - FX_DIV_R, X, S, R);
-      FX_PLOOP { A[p] = t_div(A[p], R[p]); }
+      FX_PLOOP { A[p] = fx_slow_div(A[p], R[p]); }
     } else if (op >= FX_RDIV_R && op < FX_RDIV_R + FX_NR) {
       T R[P];
       FX_PLOOP { R[p] = A[p]; }
       fx_reg_dyn<T, NX, P>(op - FX_RDIV_R, X, S, R);
-      FX_PLOOP { A[p] = t_div(R[p], A[p]); }
+      FX_PLOOP { A[p] = fx_slow_div(R[p], A[p]); }
     } else {
       return;  // FX_END (or an opcode naming a variable this kernel does not have)
     }

@@ -12,7 +12,11 @@
 #define FX_WANT(is_cplx, nx, p) ((nx) == FX_N && (p) == 2)  // real (deformation program) and complex, P = 2
 #include "fx_device_common.cuh"
 
-namespace {
+#define FX_CAT2(a, b) a##b
+#define FX_CAT(a, b) FX_CAT2(a, b)
+
+// one named namespace per dimension: the objects of all dimensions are linked into one library
+namespace FX_CAT(fx_cplx_n, FX_N) {
 
 constexpr int N = FX_N;
 constexpr int P = FX_P_CPLX;
@@ -130,6 +134,7 @@ struct IntegrateSinkCplx {
   }
 };
 
+template <int RULE>
 __global__ void __launch_bounds__(FX_THREADS) fx_integrate_cplx(const __grid_constant__ fx_integrate_params prm) {
   extern __shared__ __align__(16) unsigned char smem[];
   const int b = blockIdx.x;
@@ -138,7 +143,7 @@ __global__ void __launch_bounds__(FX_THREADS) fx_integrate_cplx(const __grid_con
   const int sel_idx = b / (prm.nchunks * prm.n_shifts);
   const fx_sector_dev sec = prm.sectors[prm.sel[sel_idx]];
   if (!sec.is_complex) return;
-  const bool vegas = prm.rule == FIESTA_RULE_VEGAS;
+  constexpr bool vegas = RULE == FIESTA_RULE_VEGAS;
   const fx_smem_layout L = fx_layout(prm.prog_ins_max, prm.mem_doubles, N, prm.nbins, vegas);
   fx_ins *sh_prog = reinterpret_cast<fx_ins *>(smem + L.prog);
   fx_ins *sh_deform = sec.deform_len ? sh_prog + sec.main_len : nullptr;
@@ -165,7 +170,7 @@ __global__ void __launch_bounds__(FX_THREADS) fx_integrate_cplx(const __grid_con
     double x[N][P], xbar[N][P], W[P], h2[P];
     uint32_t bins[(N + 3) / 4][P];
     unsigned valid;
-    fx_make_points<N, P>(prm, N, (uint32_t)sec.sector_id, sh_delta, sh_grid, base, c1, x, xbar, W, valid, bins);
+    fx_make_points<RULE, N, P>(prm, N, (uint32_t)sec.sector_id, sh_delta, sh_grid, base, c1, x, xbar, W, valid, bins);
     cplx X[N][P], Wd[P];
     fx_deform_points(sh_deform, sec.lambda, x, xbar, Mr, X, Wd);
     FX_PLOOP {
@@ -238,15 +243,21 @@ __global__ void __launch_bounds__(FX_THREADS) fx_eval_cplx(const __grid_constant
 }
 
 }  // namespace
-
-#define FX_CAT2(a, b) a##b
-#define FX_CAT(a, b) FX_CAT2(a, b)
+using namespace FX_CAT(fx_cplx_n, FX_N);
 
 cudaError_t FX_CAT(fx_launch_integrate_cplx_n, FX_N)(const fx_integrate_params &prm, size_t smem, cudaStream_t st) {
-  cudaError_t e = cudaFuncSetAttribute(fx_integrate_cplx, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return e;
   const unsigned grid = (unsigned)((size_t)prm.nsel * prm.n_shifts * prm.nchunks);
-  fx_integrate_cplx<<<grid, FX_THREADS, smem, st>>>(prm);
+  cudaError_t e;
+#define FX_LAUNCH(RULE)                                                                                                \
+  {                                                                                                                    \
+    e = cudaFuncSetAttribute(fx_integrate_cplx<RULE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);         \
+    if (e != cudaSuccess) return e;                                                                                    \
+    fx_integrate_cplx<RULE><<<grid, FX_THREADS, smem, st>>>(prm);                                                        \
+  }
+  if (prm.rule == FIESTA_RULE_LATTICE) FX_LAUNCH(FIESTA_RULE_LATTICE)
+  else if (prm.rule == FIESTA_RULE_MC) FX_LAUNCH(FIESTA_RULE_MC)
+  else FX_LAUNCH(FIESTA_RULE_VEGAS)
+#undef FX_LAUNCH
   return cudaGetLastError();
 }
 

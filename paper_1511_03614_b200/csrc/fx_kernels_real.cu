@@ -29,8 +29,8 @@ struct IntegrateSinkReal {
   }
 };
 
-template <int NX>
-__global__ void __launch_bounds__(FX_THREADS) fx_integrate_real(const __grid_constant__ fx_integrate_params prm) {
+template <int NX, int RULE>
+__global__ void __launch_bounds__(FX_THREADS, NX <= 8 ? 3 : 2) fx_integrate_real(const __grid_constant__ fx_integrate_params prm) {
   constexpr int P = FX_P_REAL;
   extern __shared__ __align__(16) unsigned char smem[];
   const int b = blockIdx.x;
@@ -40,7 +40,7 @@ __global__ void __launch_bounds__(FX_THREADS) fx_integrate_real(const __grid_con
   const fx_sector_dev sec = prm.sectors[prm.sel[sel_idx]];
   if (sec.is_complex) return;
   const int dim = prm.dim;
-  const bool vegas = prm.rule == FIESTA_RULE_VEGAS;
+  constexpr bool vegas = RULE == FIESTA_RULE_VEGAS;
   const fx_smem_layout L = fx_layout(prm.prog_ins_max, prm.mem_doubles, dim, prm.nbins, vegas);
   fx_ins *sh_prog = reinterpret_cast<fx_ins *>(smem + L.prog);
   double *sh_mem = reinterpret_cast<double *>(smem + L.mem);
@@ -64,7 +64,7 @@ __global__ void __launch_bounds__(FX_THREADS) fx_integrate_real(const __grid_con
     double x[NX][P], xbar[NX][P], W[P], h2[P];
     uint32_t bins[(NX + 3) / 4][P];
     unsigned valid;
-    fx_make_points<NX, P>(prm, dim, (uint32_t)sec.sector_id, sh_delta, sh_grid, base, c1, x, xbar, W, valid, bins);
+    fx_make_points<RULE, NX, P>(prm, dim, (uint32_t)sec.sector_id, sh_delta, sh_grid, base, c1, x, xbar, W, valid, bins);
     FX_PLOOP { h2[p] = 0.0; }
     IntegrateSinkReal<P> sink{sh_acc + threadIdx.x, W, valid, 0u, h2};
     fx_run<double, NX, P>(sh_prog, x, M, sink);
@@ -139,15 +139,22 @@ cudaError_t fx_launch_integrate_real(const fx_integrate_params &prm, cudaStream_
   const size_t smem = fx_integrate_smem_bytes(prm);
   const unsigned grid = (unsigned)((size_t)prm.nsel * prm.n_shifts * prm.nchunks);
   cudaError_t e;
-#define FX_LAUNCH(NX)                                                             \
-  {                                                                               \
-    if ((e = set_smem(fx_integrate_real<NX>, smem)) != cudaSuccess) return e;     \
-    fx_integrate_real<NX><<<grid, FX_THREADS, smem, st>>>(prm);                     \
+#define FX_LAUNCH2(NX, RULE)                                                            \
+  {                                                                                     \
+    if ((e = set_smem(fx_integrate_real<NX, RULE>, smem)) != cudaSuccess) return e;     \
+    fx_integrate_real<NX, RULE><<<grid, FX_THREADS, smem, st>>>(prm);                     \
+  }
+#define FX_LAUNCH(NX)                                                  \
+  {                                                                    \
+    if (prm.rule == FIESTA_RULE_LATTICE) FX_LAUNCH2(NX, FIESTA_RULE_LATTICE) \
+    else if (prm.rule == FIESTA_RULE_MC) FX_LAUNCH2(NX, FIESTA_RULE_MC)      \
+    else FX_LAUNCH2(NX, FIESTA_RULE_VEGAS)                                   \
   }
   if (prm.dim <= 4) FX_LAUNCH(4)
   else if (prm.dim <= 8) FX_LAUNCH(8)
   else FX_LAUNCH(12)
 #undef FX_LAUNCH
+#undef FX_LAUNCH2
   return cudaGetLastError();
 }
 
