@@ -10,7 +10,7 @@
 #include "fx_kernels.h"
 
 struct fx_smem_layout {
-  uint32_t prog, mem, acc, delta, grid, hist, wsum, total;
+  uint32_t prog, mem, acc, delta, tf, grid, hist, wsum, total;
 };
 
 __host__ __device__ inline fx_smem_layout fx_layout(int prog_ins, int mem_doubles, int dim, int nbins, bool vegas) {
@@ -24,6 +24,8 @@ __host__ __device__ inline fx_smem_layout fx_layout(int prog_ins, int mem_double
   o += FX_ACC_SLOTS * FX_THREADS * 8u;
   L.delta = o;
   o += FX_NXMAX * 8u;
+  L.tf = o;
+  o += 80u;  // fx_transform (72 bytes), kept in shared memory for the per-coordinate helper
   L.grid = o;
   o += vegas ? (uint32_t)dim * (nbins + 1) * 8u : 0u;
   L.hist = o;
@@ -50,9 +52,10 @@ struct fx_tpair {
   uint64_t e, o;
 };
 
-static __device__ __noinline__ fx_coord fx_lattice_coord(uint64_t t, const fx_transform *tf) {
+static __device__ __noinline__ fx_coord fx_lattice_coord(uint64_t t, const fx_transform *tf /* shared memory */) {
   fx_coord c;
-  korobov_transform(*tf, unit_from_t(t), c.x, c.xbar, c.w);
+  if (tf->r == 3) korobov_transform_r<3>(*tf, unit_from_t(t), c.x, c.xbar, c.w);  // the default weight: no switch
+  else korobov_transform(*tf, unit_from_t(t), c.x, c.xbar, c.w);
   return c;
 }
 
@@ -88,7 +91,7 @@ __device__ __forceinline__ void fx_make_points(const fx_integrate_params &prm, i
 #pragma unroll
   for (int q = 0; q < (NX + 3) / 4; ++q) FX_PLOOP { bins[q][p] = 0; }
   if constexpr (RULE == FIESTA_RULE_LATTICE) {
-    const fx_transform *tf = reinterpret_cast<const fx_transform *>(&prm.tf);
+    const fx_transform *tf = reinterpret_cast<const fx_transform *>(sh_delta + FX_NXMAX);  // fx_layout: tf follows delta
 #pragma unroll
     for (int k = 0; k < NX; ++k) {
       if (k < dim) {
@@ -150,6 +153,12 @@ __device__ __forceinline__ void fx_block_setup(const fx_integrate_params &prm, i
       philox_t_pair(prm.seed, sector_id, FX_TAG_SHIFT, (uint32_t)r, 0ull, threadIdx.x, te, to);
     sh_delta[2 * threadIdx.x] = te;
     sh_delta[2 * threadIdx.x + 1] = to;
+  }
+  if (threadIdx.x == 32) {  // fx_layout puts the transform right after the shifts
+    fx_transform *tf = reinterpret_cast<fx_transform *>(sh_delta + FX_NXMAX);
+    tf->r = prm.tf.r;
+    tf->cw = prm.tf.cw;
+    for (int i = 0; i < 7; ++i) tf->coef[i] = prm.tf.coef[i];
   }
   if (prm.rule == FIESTA_RULE_VEGAS) {
     const double *g = prm.grid + (size_t)sel_idx * dim * (prm.nbins + 1);

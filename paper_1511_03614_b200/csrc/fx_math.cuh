@@ -152,28 +152,47 @@ struct fx_transform {
   double coef[7]; // phi_r(v) = v^(r+1) * sum_i coef[i] v^i
 };
 
-__device__ __forceinline__ void korobov_transform(const fx_transform &tf, double u, double &x, double &xbar,
-                                                  double &w) {
-  double ubar = 1.0 - u;  // exact: u is an odd multiple of 2^-53
-  if (tf.r == 0) {
+template <int R>
+__device__ __forceinline__ void korobov_transform_r(const fx_transform &tf, double u, double &x, double &xbar,
+                                                    double &w) {
+  const double ubar = 1.0 - u;  // exact: u is an odd multiple of 2^-53
+  if constexpr (R == 0) {
     x = u;
     xbar = ubar;
     w = 1.0;
-    return;
+  } else {
+    const double v = fmin(u, ubar);
+    double poly = tf.coef[R];
+#pragma unroll
+    for (int i = R - 1; i >= 0; --i) poly = fma(poly, v, tf.coef[i]);
+    double vp = v;
+#pragma unroll
+    for (int i = 0; i < R; ++i) vp *= v;
+    const double p = vp * poly;
+    const double big = 1.0 - p;
+    const bool left = u <= ubar;
+    x = left ? p : big;
+    xbar = left ? big : p;
+    const double s = u * ubar;
+    double sp = s;
+#pragma unroll
+    for (int i = 1; i < R; ++i) sp *= s;
+    w = tf.cw * sp;
   }
-  double v = fmin(u, ubar);
-  double poly = tf.coef[tf.r];
-  for (int i = tf.r - 1; i >= 0; --i) poly = fma(poly, v, tf.coef[i]);
-  double vp = v;
-  for (int i = 0; i < tf.r; ++i) vp *= v;
-  double p = vp * poly;
-  double big = 1.0 - p;
-  bool left = u <= ubar;
-  x = left ? p : big;
-  xbar = left ? big : p;
-  double s = u * ubar, sp = s;
-  for (int i = 1; i < tf.r; ++i) sp *= s;
-  w = tf.cw * sp;
+}
+
+// run-time weight: same arithmetic, in the same order, for every r
+__device__ __forceinline__ void korobov_transform(const fx_transform &tf, double u, double &x, double &xbar,
+                                                  double &w) {
+  switch (tf.r) {
+    case 0: korobov_transform_r<0>(tf, u, x, xbar, w); break;
+    case 1: korobov_transform_r<1>(tf, u, x, xbar, w); break;
+    case 2: korobov_transform_r<2>(tf, u, x, xbar, w); break;
+    case 3: korobov_transform_r<3>(tf, u, x, xbar, w); break;
+    case 4: korobov_transform_r<4>(tf, u, x, xbar, w); break;
+    case 5: korobov_transform_r<5>(tf, u, x, xbar, w); break;
+    default: korobov_transform_r<6>(tf, u, x, xbar, w); break;
+  }
 }
 
 // Vegas map of one coordinate (R8): exact integer bin and fraction, then the edges.
