@@ -574,67 +574,82 @@ struct Emitter {
     if (o.kind == Opnd::REG) sfree[o.idx - FX_NXMAX] = true;
     else if (o.kind == Opnd::MEM) mfree.push_back(o.idx);
   }
-  void store(const Opnd &o) {
-    if (o.kind == Opnd::REG) ins(FX_ST_S + (o.idx - FX_NXMAX));
-    else ins(FX_STM, o.idx);
+  int lvl = 0;  // accumulator level the arithmetic helpers act on (0 outside horner())
+  int LR(int base, const Opnd &o) const { return base + lvl * FX_NR + o.idx; }
+  Opnd alloc_mem_temp() {
+    Opnd o;
+    o.kind = Opnd::MEM;
+    if (!mfree.empty()) {
+      o.idx = mfree.back();
+      mfree.pop_back();
+    } else {
+      o.idx = mhigh++;
+      if (mhigh > 4096) fail(FIESTA_E_TOOBIG, "expression needs more than 4096 spill slots");
+    }
+    return o;
   }
-  // -- A <op> operand helpers
+  void store(const Opnd &o) {  // from level 0 (registers) or any level (memory)
+    if (o.kind == Opnd::REG) {
+      if (lvl != 0) fail(FIESTA_E_ARG, "internal: register store from a nested level");
+      ins(FX_ST_S + (o.idx - FX_NXMAX));
+    } else
+      ins(FX_STM + lvl, o.idx);
+  }
+  // -- A[lvl] <op> operand helpers
   void load(const Opnd &o) {
-    if (o.kind == Opnd::IMM) ins(FX_LDC, 0, o.c);
-    else if (o.kind == Opnd::REG) ins(FX_LD_R + o.idx);
-    else ins(FX_LDM, o.idx);
+    if (o.kind == Opnd::IMM) ins(FX_LDC + lvl, 0, o.c);
+    else if (o.kind == Opnd::REG) ins(LR(FX_LD_R, o));
+    else ins(FX_LDM + lvl, o.idx);
   }
   void mul(const Opnd &o) {
     if (o.kind == Opnd::IMM) {
-      if (o.c != 1.0) ins(FX_MULC, 0, o.c);
-    } else if (o.kind == Opnd::REG) ins(FX_MUL_R + o.idx);
-    else ins(FX_MULM, o.idx);
+      if (o.c != 1.0) ins(FX_MULC + lvl, 0, o.c);
+    } else if (o.kind == Opnd::REG) ins(LR(FX_MUL_R, o));
+    else ins(FX_MULM + lvl, o.idx);
   }
   void add(const Opnd &o) {
     if (o.kind == Opnd::IMM) {
-      if (o.c != 0.0) ins(FX_ADDC, 0, o.c);
-    } else if (o.kind == Opnd::REG) ins(FX_ADD_R + o.idx);
-    else ins(FX_ADDM, o.idx);
+      if (o.c != 0.0) ins(FX_ADDC + lvl, 0, o.c);
+    } else if (o.kind == Opnd::REG) ins(LR(FX_ADD_R, o));
+    else ins(FX_ADDM + lvl, o.idx);
   }
-  void div(const Opnd &o) {  // A = A / o
+  void div(const Opnd &o) {  // A = A / o   (level 0)
     if (o.kind == Opnd::IMM) ins(FX_DIVC, 0, o.c);
     else if (o.kind == Opnd::REG) ins(FX_DIV_R + o.idx);
     else ins(FX_DIVM, o.idx);
   }
-  void rdiv(const Opnd &o) {  // A = o / A
+  void rdiv(const Opnd &o) {  // A = o / A   (level 0)
     if (o.kind == Opnd::IMM) ins(FX_RDIVC, 0, o.c);
     else if (o.kind == Opnd::REG) ins(FX_RDIV_R + o.idx);
     else ins(FX_RDIVM, o.idx);
   }
   void fma_a(const Opnd &m, const Opnd &addend) {  // A = A*m + addend ; m is REG or MEM
     if (m.kind == Opnd::REG) {
-      if (addend.kind == Opnd::IMM) ins(FX_FMA_AR_C + m.idx, 0, addend.c);
-      else if (addend.kind == Opnd::REG && addend.idx >= FX_NXMAX)
-        ins(FX_FMA_AR_S + m.idx * FX_NS + (addend.idx - FX_NXMAX));
-      else if (addend.kind == Opnd::MEM) ins(FX_FMA_AR_M + m.idx, addend.idx);
+      if (addend.kind == Opnd::IMM) ins(LR(FX_FMA_AR_C, m), 0, addend.c);
+      else if (addend.kind == Opnd::MEM) ins(LR(FX_FMA_AR_M, m), addend.idx);
       else {
-        ins(FX_MUL_R + m.idx);
+        ins(LR(FX_MUL_R, m));
         add(addend);
       }
     } else {
-      if (addend.kind == Opnd::IMM) ins(FX_FMA_AM_C, m.idx, addend.c);
+      if (addend.kind == Opnd::IMM) ins(FX_FMA_AM_C + lvl, m.idx, addend.c);
       else {
-        ins(FX_MULM, m.idx);
+        ins(FX_MULM + lvl, m.idx);
         add(addend);
       }
     }
   }
   void fma_into_a(const Opnd &m, double c) {  // A = m*c + A
-    if (m.kind == Opnd::REG) ins(FX_FMA_RC_A + m.idx, 0, c);
-    else ins(FX_FMA_MC_A, m.idx, c);
+    if (m.kind == Opnd::REG) ins(LR(FX_FMA_RC_A, m), 0, c);
+    else ins(FX_FMA_MC_A + lvl, m.idx, c);
   }
   void mulc_load(const Opnd &m, double c) {  // A = c*m
     if (m.kind == Opnd::REG) {
-      if (c == 1.0) ins(FX_LD_R + m.idx);
-      else ins(FX_MULC_R + m.idx, 0, c);
+      if (c == 1.0) ins(LR(FX_LD_R, m));
+      else ins(LR(FX_MULC_R, m), 0, c);
     } else {
-      ins(FX_LDM, m.idx);
-      if (c != 1.0) ins(FX_MULC, 0, c);
+      ins(FX_LDM + lvl, m.idx);
+      if (c != 1.0) ins(FX_MULC + lvl, 0, c);
     }
   }
 
@@ -809,13 +824,13 @@ struct Emitter {
   // Greedy multivariate Horner: p = v*q + r with v the atom that divides most terms.
   void horner(const Poly &terms) {
     if (terms.empty()) {
-      ins(FX_LDC, 0, 0.0);
+      ins(FX_LDC + lvl, 0, 0.0);
       return;
     }
     if (terms.size() == 1) {
       const Term &t = terms[0];
       if (t.f.empty()) {
-        ins(FX_LDC, 0, t.c);
+        ins(FX_LDC + lvl, 0, t.c);
         return;
       }
       bool started = false;
@@ -881,8 +896,23 @@ struct Emitter {
       fma_into_a(operand_of(r[0].f[0].first), r[0].c);
       return;
     }
+    // general case p = q*v + r: r stays in A[lvl] while q is evaluated one level up, then one
+    // FMA folds them -- no store/reload of the partial result
     horner(r);
-    Opnd t = alloc_temp();
+    if (lvl + 1 < FX_L) {
+      ++lvl;
+      horner(q);
+      if (vo.kind == Opnd::REG) {
+        --lvl;
+        ins(LR(FX_FMA_UP, vo));
+      } else {
+        mul(vo);
+        --lvl;
+        ins(FX_ADD_UP + lvl);
+      }
+      return;
+    }
+    Opnd t = alloc_mem_temp();  // nesting deeper than the accumulator stack: spill r to shared memory
     store(t);
     horner(q);
     fma_a(vo, t);
@@ -890,15 +920,19 @@ struct Emitter {
   }
 };
 
+namespace {
+bool in_fam(int op, int base, int n) { return op >= base && op < base + n; }
+}
+
 void fill_info(const std::vector<fx_ins> &code, fiesta_compile_info &info) {
   for (auto &i : code) {
     int op = i.op;
     if (op == FX_END) continue;
     info.n_ir_ops++;
-    bool fma = (op < FX_MUL_R) || (op >= FX_FMA_AR_M && op < FX_ST_S) || op == FX_FMA_AM_C || op == FX_FMA_MC_A;
-    bool div = (op >= FX_DIV_R && op < FX_FMA_AR_M) || op == FX_DIVC || op == FX_RDIVC || op == FX_DIVM || op == FX_RDIVM;
-    bool move = (op >= FX_LD_R && op < FX_MULC_R) || (op >= FX_ST_S && op < FX_LDC) || op == FX_LDC || op == FX_LDM ||
-                op == FX_STM || op == FX_OUT || op == FX_NEG;
+    bool fma = in_fam(op, FX_FMA_AR_C, 3 * FX_LR) || in_fam(op, FX_FMA_AR_M, FX_LR) || in_fam(op, FX_FMA_MC_A, 2 * FX_L);
+    bool div = in_fam(op, FX_DIV_R, 2 * FX_NR) || op == FX_DIVC || op == FX_RDIVC || op == FX_DIVM || op == FX_RDIVM;
+    bool move = in_fam(op, FX_LD_R, FX_LR) || in_fam(op, FX_ST_S, FX_NS) || in_fam(op, FX_LDC, FX_L) ||
+                in_fam(op, FX_LDM, 2 * FX_L) || op == FX_OUT || op == FX_NEG;
     if (move) continue;
     info.n_fp64_ops++;
     if (fma) {
@@ -1076,31 +1110,32 @@ CompiledSector compile_sector(const char *const *texts, int K, int dim, bool is_
 }
 
 std::string disassemble(const std::vector<fx_ins> &prog) {
-  static const char *fam[] = {"A=A*R%d+%g", "A=R%d*%g+A", "A=A*R%d", "A=A+R%d", "A=A-R%d", "A=R%d-A",
-                              "A=R%d", "A=%2$g*R%1$d", "A=A/R%d", "A=R%d/A"};
-  static const char *single[] = {"A=imm", "A=A+imm", "A=A*imm", "A=imm-A", "A=A/imm", "A=imm/A", "A=M", "M=A",
-                                 "A=A+M", "A=A-M", "A=M-A", "A=A*M", "A=A/M", "A=M/A", "A=A*M+imm", "A=M*imm+A",
-                                 "A=-A", "A=A*A", "A=log A", "A=exp A", "A=sqrt A", "OUT", "END"};
+  static const char *lr[] = {"A%d=%3$g*R%2$d", "A%d*=R%d", "A%d=A%1$d*R%d+%g", "A%d+=R%d*%g", "A%d+=A[+1]*R%d",
+                             "A%d+=R%d", "A%d=R%d", "A%d=A%1$d*R%d+M"};
+  static const char *lv[] = {"A%d=imm", "A%d+=imm", "A%d*=imm", "A%d+=A[+1]", "A%d*=A[+1]", "A%d=M", "M=A%d",
+                             "A%d+=M", "A%d*=M", "A%d+=M*imm", "A%d=A%1$d*M+imm"};
+  static const char *r0[] = {"A-=R%d", "A=R%d-A", "A/=R%d", "A=R%d/A"};
+  static const char *single[] = {"A=imm-A", "A/=imm", "A=imm/A", "A-=M", "A=M-A", "A/=M", "A=M/A", "A=-A", "A=A*A",
+                                 "A=log A", "A=exp A", "A=sqrt A", "OUT", "END"};
   std::string out;
-  char buf[160];
+  char buf[200], b2[120];
   for (size_t pc = 0; pc < prog.size(); ++pc) {
     const fx_ins &i = prog[pc];
     int op = i.op;
-    if (op < FX_FMA_AR_M) {
-      int f = op / FX_NR, r = op % FX_NR;
-      char b2[96];
-      std::snprintf(b2, sizeof b2, fam[f], r, i.imm);
-      std::snprintf(buf, sizeof buf, "%4zu  %s\n", pc, b2);
-    } else if (op < FX_FMA_AR_S) {
-      std::snprintf(buf, sizeof buf, "%4zu  A=A*R%d+M[%d]\n", pc, op - FX_FMA_AR_M, i.aux);
+    if (op < FX_LDC) {
+      int f = op / FX_LR, d = (op % FX_LR) / FX_NR, r = op % FX_NR;
+      std::snprintf(b2, sizeof b2, lr[f], d, r, i.imm);
+    } else if (op < FX_SUB_R) {
+      int f = (op - FX_LDC) / FX_L, d = (op - FX_LDC) % FX_L;
+      std::snprintf(b2, sizeof b2, lv[f], d);
     } else if (op < FX_ST_S) {
-      int x = op - FX_FMA_AR_S;
-      std::snprintf(buf, sizeof buf, "%4zu  A=A*R%d+S%d\n", pc, x / FX_NS, x % FX_NS);
-    } else if (op < FX_LDC) {
-      std::snprintf(buf, sizeof buf, "%4zu  S%d=A\n", pc, op - FX_ST_S);
+      std::snprintf(b2, sizeof b2, r0[(op - FX_SUB_R) / FX_NR], (op - FX_SUB_R) % FX_NR);
+    } else if (op < FX_RSUBC) {
+      std::snprintf(b2, sizeof b2, "S%d=A", op - FX_ST_S);
     } else {
-      std::snprintf(buf, sizeof buf, "%4zu  %s  aux=%d imm=%.17g\n", pc, single[op - FX_LDC], i.aux, i.imm);
+      std::snprintf(b2, sizeof b2, "%s", single[op - FX_RSUBC]);
     }
+    std::snprintf(buf, sizeof buf, "%4zu  %-22s aux=%d imm=%.17g\n", pc, b2, i.aux, i.imm);
     out += buf;
   }
   return out;

@@ -76,16 +76,18 @@ __device__ __forceinline__ void fx_reg_dyn(int r, const T (&X)[NX][P], const T (
 // output k (FX_OUT).  M are this thread's spill slots (stride must be FX_THREADS).
 template <typename T, int NX, int P, class Sink>
 __device__ __forceinline__ void fx_run(const fx_ins *prog, T (&X)[NX][P], const fx_mem<T> M, Sink &sink) {
-  T A[P];
+  T AL[FX_L][P];  // accumulator levels; the slow path only ever touches level 0
   T S[FX_NS][P];
-  FX_PLOOP { A[p] = t_from_real(0.0, T{}); }
+#pragma unroll
+  for (int d = 0; d < FX_L; ++d) FX_PLOOP { AL[d][p] = t_from_real(0.0, T{}); }
 #pragma unroll
   for (int j = 0; j < FX_NS; ++j) FX_PLOOP { S[j][p] = t_from_real(0.0, T{}); }
+  T(&A)[P] = AL[0];
   uint32_t pc = (uint32_t)__cvta_generic_to_shared(prog);
   const uint32_t mem = (uint32_t)__cvta_generic_to_shared(M.base);
   for (;;) {
     uint32_t w0, w2, w3;
-    fx_fast<T, NX, P>::run(A, X, S, pc, mem, w0, w2, w3);
+    fx_fast<T, NX, P>::run(AL, X, S, pc, mem, w0, w2, w3);
     const int op = w0 & 0xffff;
     const int aux = w0 >> 16;
     const double imm = __hiloint2double((int)w3, (int)w2);

@@ -31,11 +31,20 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 THREADED = False
 PREFETCH = True
 THREADS = 128   # FX_THREADS: stride (in doubles) between spill slots of one thread
-NXMAX, NS = 12, 8
 
 
 def parse_isa():
+    """opcode names -> numbers, evaluating the `= expr` forms of fx_isa.h with its #defines."""
     txt = open(os.path.join(HERE, "fx_isa.h")).read()
+    env = {}
+    for m in re.finditer(r"^#define\s+(FX_\w+)\s+(.+?)\s*(?://.*)?$", txt, re.M):
+        name, val = m.group(1), m.group(2)
+        if "(" in name:
+            continue
+        try:
+            env[name] = int(eval(val, {}, env))
+        except Exception:
+            pass
     body = txt[txt.index("enum fx_op"):]
     body = body[body.index("{") + 1:body.index("};")]
     ops, val = {}, 0
@@ -43,18 +52,19 @@ def parse_isa():
         line = line.split("//")[0].strip().rstrip(",")
         if not line:
             continue
-        m = re.match(r"(\w+)\s*=\s*(\d+)$", line)
+        m = re.match(r"(\w+)\s*=\s*(.+)$", line)
         if m:
-            val = int(m.group(2))
+            val = int(eval(m.group(2), {}, {**env, **ops}))
             ops[m.group(1)] = val
         else:
             ops[line] = val
         val += 1
-    return ops
+    return ops, env
 
 
-OPS = parse_isa()
+OPS, ENV = parse_isa()
 NOPS = OPS["FX_NOPS"]
+NXMAX, NS, NL, NR = ENV["FX_NXMAX"], ENV["FX_NS"], ENV["FX_L"], ENV["FX_NR"]
 
 
 class Gen:
@@ -72,7 +82,8 @@ class Gen:
 
     def setup(self):
         comp = (".re", ".im") if self.cplx else ("",)
-        self.A = [[self.opnd("+d", f"A[{p}]{c}") for c in comp] for p in range(self.p)]
+        self.AL = [[[self.opnd("+d", f"A[{d}][{p}]{c}") for c in comp] for p in range(self.p)] for d in range(NL)]
+        self.A = self.AL[0]
         self.X = [[[self.opnd("+d", f"X[{k}][{p}]{c}") for c in comp] for p in range(self.p)] for k in range(self.nx)]
         self.S = [[[self.opnd("+d", f"S[{j}][{p}]{c}") for c in comp] for p in range(self.p)] for j in range(NS)]
         self.pc = self.opnd("+r", "pc")
@@ -146,6 +157,16 @@ class Gen:
         for c in range(self.C):
             self.emit(f"fma.rn.f64 {a[c]}, {r[c]}, {imm}, {a[c]};")
 
+    def fma_up(self, a, u, r):            # a = u*r + a
+        if not self.cplx:
+            self.emit(f"fma.rn.f64 {a[0]}, {u[0]}, {r[0]}, {a[0]};")
+            return
+        self.emit(f"neg.f64 t0, {u[1]};")
+        self.emit(f"fma.rn.f64 t0, t0, {r[1]}, {a[0]};")
+        self.emit(f"fma.rn.f64 {a[0]}, {u[0]}, {r[0]}, t0;")
+        self.emit(f"fma.rn.f64 t1, {u[1]}, {r[0]}, {a[1]};")
+        self.emit(f"fma.rn.f64 {a[1]}, {u[0]}, {r[1]}, t1;")
+
     def mul(self, a, b):                  # a = a*b
         if not self.cplx:
             self.emit(f"mul.rn.f64 {a[0]}, {a[0]}, {b[0]};")
@@ -167,19 +188,17 @@ class Gen:
         so that their union stays inside the 32 KB L1.5 instruction cache (the first layout spread
         them over 87 KB: icc hit rate 60 %, 'no instruction' the top stall)."""
         m = re.match(r"H_([A-Z_]+?)(?:_(\d+))?(?:_(\d+))?$", label)
-        fam, r = m.group(1), m.group(2)
-        isx = r is not None and int(r) < NXMAX
-        if fam in ("FMA_AR_C", "FMA_RC_A", "MUL_R", "MULC_R") and isx:
+        fam = m.group(1)
+        nums = [int(g) for g in m.groups()[1:] if g is not None]
+        r = nums[-1] if len(nums) == 2 else None
+        isx = r is not None and r < NXMAX
+        if fam in ("MULC_R", "MUL_R", "FMA_AR_C", "FMA_RC_A", "FMA_UP") and isx:
             return 0
-        if fam == "ST_S":
-            return 0
-        if fam == "FMA_AR_S" and isx:
-            return 1
-        if fam in ("LDC", "ADDC", "MULC", "NEG", "SQR", "RSUBC"):
+        if fam in ("LDC", "ADDC", "MULC", "ADD_UP", "MUL_UP", "ST_S", "NEG", "SQR", "RSUBC"):
             return 1
         if "DIV" in fam or fam == "SQRT":
             return 9
-        if fam.endswith("M") or "_AM_" in fam or "_MC_" in fam:
+        if fam.endswith("M") or "_AM_" in fam or "_MC_" in fam or fam == "FMA_AR_M":
             return 5
         return 2 if isx else 3
 
@@ -198,38 +217,71 @@ class Gen:
     def build(self):
         self.setup()
         table = ["EXIT"] * NOPS
-        A, cx = self.A, self.cplx
+        AL, cx, C = self.AL, self.cplx, self.C
 
-        def reg_family(base, name, body, ok=True):
-            for r in range(NXMAX + NS):
-                if not ok or (r < NXMAX and r >= self.nx):
-                    continue
-                lab = f"H_{name}_{r}"
-                table[OPS[base] + r] = lab
-                self.handler(lab, lambda p, r=r: body(A[p], self.R(r)[p], p), pre=self.mem_addr if name == "FMA_AR_M" else None)
+        def regs():
+            return [r for r in range(NR) if not (r < NXMAX and r >= self.nx)]
 
-        reg_family("FX_FMA_AR_C", "FMA_AR_C", lambda a, r, p: self.fma_c(a, r))
-        reg_family("FX_FMA_RC_A", "FMA_RC_A", lambda a, r, p: self.fma_rc(a, r))
-        reg_family("FX_MUL_R", "MUL_R", lambda a, r, p: self.mul(a, r))
-        reg_family("FX_ADD_R", "ADD_R", lambda a, r, p: self.comp2("add.rn.f64", a, a, r))
-        reg_family("FX_SUB_R", "SUB_R", lambda a, r, p: self.comp2("sub.rn.f64", a, a, r))
-        reg_family("FX_RSUB_R", "RSUB_R", lambda a, r, p: self.comp2("sub.rn.f64", a, r, a))
-        reg_family("FX_LD_R", "LD_R", lambda a, r, p: [self.emit(f"mov.f64 {a[c]}, {r[c]};") for c in range(self.C)])
-        reg_family("FX_MULC_R", "MULC_R", lambda a, r, p: [self.emit(f"mul.rn.f64 {a[c]}, {r[c]}, imm;") for c in range(self.C)])
-        reg_family("FX_DIV_R", "DIV_R", lambda a, r, p: self.emit(f"div.rn.f64 {a[0]}, {a[0]}, {r[0]};"), ok=not cx)
-        reg_family("FX_RDIV_R", "RDIV_R", lambda a, r, p: self.emit(f"div.rn.f64 {a[0]}, {r[0]}, {a[0]};"), ok=not cx)
-        reg_family("FX_FMA_AR_M", "FMA_AR_M", lambda a, r, p: self.fma_full(a, r, self.ld_mem(p)))
-        for r in range(NXMAX + NS):
-            if r < NXMAX and r >= self.nx:
-                continue
-            for j in range(NS):
-                lab = f"H_FMA_AR_S_{r}_{j}"
-                table[OPS["FX_FMA_AR_S"] + r * NS + j] = lab
-                self.handler(lab, lambda p, r=r, j=j: self.fma_full(A[p], self.R(r)[p], self.S[j][p]))
+        def lr_family(name, body, pre=None, dmax=NL):
+            """opcode = base + d*NR + r; body(a, r, d, p)"""
+            for d in range(dmax):
+                for r in regs():
+                    lab = f"H_{name}_{d}_{r}"
+                    table[OPS["FX_" + name] + d * NR + r] = lab
+                    self.handler(lab, lambda p, d=d, r=r: body(AL[d][p], self.R(r)[p], d, p), pre)
+
+        def l_family(name, body, pre=None, dmax=NL):
+            """opcode = base + d; body(a, d, p)"""
+            for d in range(dmax):
+                lab = f"H_{name}_{d}"
+                table[OPS["FX_" + name] + d] = lab
+                self.handler(lab, lambda p, d=d: body(AL[d][p], d, p), pre)
+
+        def r0_family(name, body, ok=True):
+            if not ok:
+                return
+            for r in regs():
+                lab = f"H_{name}_0_{r}"
+                table[OPS["FX_" + name] + r] = lab
+                self.handler(lab, lambda p, r=r: body(AL[0][p], self.R(r)[p], p))
+
+        E = self.emit
+        lr_family("MULC_R", lambda a, r, d, p: [E(f"mul.rn.f64 {a[c]}, {r[c]}, imm;") for c in range(C)])
+        lr_family("MUL_R", lambda a, r, d, p: self.mul(a, r))
+        lr_family("FMA_AR_C", lambda a, r, d, p: self.fma_c(a, r))
+        lr_family("FMA_RC_A", lambda a, r, d, p: self.fma_rc(a, r))
+        lr_family("FMA_UP", lambda a, r, d, p: self.fma_up(a, AL[d + 1][p], r), dmax=NL - 1)
+        lr_family("ADD_R", lambda a, r, d, p: self.comp2("add.rn.f64", a, a, r))
+        lr_family("LD_R", lambda a, r, d, p: [E(f"mov.f64 {a[c]}, {r[c]};") for c in range(C)])
+        lr_family("FMA_AR_M", lambda a, r, d, p: self.fma_full(a, r, self.ld_mem(p)), pre=self.mem_addr)
+
+        def ldc(a, d, p):
+            E(f"mov.f64 {a[0]}, imm;")
+            if cx:
+                E(f"mov.f64 {a[1]}, zero;")
+
+        l_family("LDC", ldc)
+        l_family("ADDC", lambda a, d, p: E(f"add.rn.f64 {a[0]}, {a[0]}, imm;"))
+        l_family("MULC", lambda a, d, p: [E(f"mul.rn.f64 {a[c]}, {a[c]}, imm;") for c in range(C)])
+        l_family("ADD_UP", lambda a, d, p: self.comp2("add.rn.f64", a, a, AL[d + 1][p]), dmax=NL - 1)
+        l_family("MUL_UP", lambda a, d, p: self.mul(a, AL[d + 1][p]), dmax=NL - 1)
+        l_family("LDM", lambda a, d, p: [E(f"mov.f64 {a[c]}, {m};") for c, m in enumerate(self.ld_mem(p))], self.mem_addr)
+        l_family("STM", lambda a, d, p: [E(f"st.shared.f64 [ma+{self.mem_off(p, c)}], {a[c]};") for c in range(C)],
+                 self.mem_addr)
+        l_family("ADDM", lambda a, d, p: self.comp2("add.rn.f64", a, a, self.ld_mem(p)), self.mem_addr)
+        l_family("MULM", lambda a, d, p: self.mul(a, self.ld_mem(p)), self.mem_addr)
+        l_family("FMA_MC_A", lambda a, d, p: self.fma_rc(a, self.ld_mem(p)), self.mem_addr)
+        l_family("FMA_AM_C", lambda a, d, p: self.fma_c(a, self.ld_mem(p)), self.mem_addr)
+
+        r0_family("SUB_R", lambda a, r, p: self.comp2("sub.rn.f64", a, a, r))
+        r0_family("RSUB_R", lambda a, r, p: self.comp2("sub.rn.f64", a, r, a))
+        r0_family("DIV_R", lambda a, r, p: E(f"div.rn.f64 {a[0]}, {a[0]}, {r[0]};"), ok=not cx)
+        r0_family("RDIV_R", lambda a, r, p: E(f"div.rn.f64 {a[0]}, {r[0]}, {a[0]};"), ok=not cx)
+        A = AL[0]
         for j in range(NS):
             lab = f"H_ST_S_{j}"
             table[OPS["FX_ST_S"] + j] = lab
-            self.handler(lab, lambda p, j=j: [self.emit(f"mov.f64 {self.S[j][p][c]}, {A[p][c]};") for c in range(self.C)])
+            self.handler(lab, lambda p, j=j: [E(f"mov.f64 {self.S[j][p][c]}, {A[p][c]};") for c in range(C)])
 
         def single(name, body, pre=None, ok=True):
             if not ok:
@@ -238,36 +290,21 @@ class Gen:
             table[OPS["FX_" + name]] = lab
             self.handler(lab, body, pre)
 
-        def ldc(p):
-            self.emit(f"mov.f64 {A[p][0]}, imm;")
-            if cx:
-                self.emit(f"mov.f64 {A[p][1]}, zero;")
-
         def rsubc(p):
-            self.emit(f"sub.rn.f64 {A[p][0]}, imm, {A[p][0]};")
+            E(f"sub.rn.f64 {A[p][0]}, imm, {A[p][0]};")
             if cx:
-                self.emit(f"neg.f64 {A[p][1]}, {A[p][1]};")
+                E(f"neg.f64 {A[p][1]}, {A[p][1]};")
 
-        single("LDC", ldc)
-        single("ADDC", lambda p: self.emit(f"add.rn.f64 {A[p][0]}, {A[p][0]}, imm;"))
-        single("MULC", lambda p: [self.emit(f"mul.rn.f64 {A[p][c]}, {A[p][c]}, imm;") for c in range(self.C)])
         single("RSUBC", rsubc)
-        single("DIVC", lambda p: [self.emit(f"div.rn.f64 {A[p][c]}, {A[p][c]}, imm;") for c in range(self.C)])
-        single("RDIVC", lambda p: self.emit(f"div.rn.f64 {A[p][0]}, imm, {A[p][0]};"), ok=not cx)
-        single("LDM", lambda p: [self.emit(f"mov.f64 {A[p][c]}, {m};") for c, m in enumerate(self.ld_mem(p))], self.mem_addr)
-        single("STM", lambda p: [self.emit(f"st.shared.f64 [ma+{self.mem_off(p, c)}], {A[p][c]};") for c in range(self.C)],
-               self.mem_addr)
-        single("ADDM", lambda p: self.comp2("add.rn.f64", A[p], A[p], self.ld_mem(p)), self.mem_addr)
+        single("DIVC", lambda p: [E(f"div.rn.f64 {A[p][c]}, {A[p][c]}, imm;") for c in range(C)])
+        single("RDIVC", lambda p: E(f"div.rn.f64 {A[p][0]}, imm, {A[p][0]};"), ok=not cx)
         single("SUBM", lambda p: self.comp2("sub.rn.f64", A[p], A[p], self.ld_mem(p)), self.mem_addr)
         single("RSUBM", lambda p: self.comp2("sub.rn.f64", A[p], self.ld_mem(p), A[p]), self.mem_addr)
-        single("MULM", lambda p: self.mul(A[p], self.ld_mem(p)), self.mem_addr)
-        single("DIVM", lambda p: self.emit(f"div.rn.f64 {A[p][0]}, {A[p][0]}, {self.ld_mem(p)[0]};"), self.mem_addr, ok=not cx)
-        single("RDIVM", lambda p: self.emit(f"div.rn.f64 {A[p][0]}, {self.ld_mem(p)[0]}, {A[p][0]};"), self.mem_addr, ok=not cx)
-        single("FMA_AM_C", lambda p: self.fma_c(A[p], self.ld_mem(p)), self.mem_addr)
-        single("FMA_MC_A", lambda p: self.fma_rc(A[p], self.ld_mem(p)), self.mem_addr)
-        single("NEG", lambda p: [self.emit(f"neg.f64 {A[p][c]}, {A[p][c]};") for c in range(self.C)])
+        single("DIVM", lambda p: E(f"div.rn.f64 {A[p][0]}, {A[p][0]}, {self.ld_mem(p)[0]};"), self.mem_addr, ok=not cx)
+        single("RDIVM", lambda p: E(f"div.rn.f64 {A[p][0]}, {self.ld_mem(p)[0]}, {A[p][0]};"), self.mem_addr, ok=not cx)
+        single("NEG", lambda p: [E(f"neg.f64 {A[p][c]}, {A[p][c]};") for c in range(C)])
         single("SQR", lambda p: self.mul(A[p], A[p]))
-        single("SQRT", lambda p: self.emit(f"sqrt.rn.f64 {A[p][0]}, {A[p][0]};"), ok=not cx)
+        single("SQRT", lambda p: E(f"sqrt.rn.f64 {A[p][0]}, {A[p][0]};"), ok=not cx)
         return table
 
     def function(self):
@@ -280,7 +317,7 @@ class Gen:
         T = "cplx" if self.cplx else "double"
         name = f"fx_fast_{kind}_{self.nx}_{self.p}"
         out = [f"#if FX_WANT({int(self.cplx)}, {self.nx}, {self.p})",
-               f"__device__ __forceinline__ void {name}({T} (&A)[{self.p}], {T} (&X)[{self.nx}][{self.p}], "
+               f"__device__ __forceinline__ void {name}({T} (&A)[{NL}][{self.p}], {T} (&X)[{self.nx}][{self.p}], "
                f"{T} (&S)[{NS}][{self.p}], uint32_t &pc, uint32_t mem, uint32_t &w0, uint32_t &w2, uint32_t &w3) {{",
                "  asm volatile(", '    "{\\n"',
                '    ".reg .u32 c0, n0, n1, n2, n3, op, ma;\\n"', '    ".reg .f64 imm, zero, t0, t1, m0, m1;\\n"',
@@ -310,7 +347,7 @@ class Gen:
         out.append('    : "memory");')
         out.append("}")
         out.append(f"template <> struct fx_fast<{T}, {self.nx}, {self.p}> {{")
-        out.append(f"  static __device__ __forceinline__ void run({T} (&A)[{self.p}], {T} (&X)[{self.nx}][{self.p}], "
+        out.append(f"  static __device__ __forceinline__ void run({T} (&A)[{NL}][{self.p}], {T} (&X)[{self.nx}][{self.p}], "
                    f"{T} (&S)[{NS}][{self.p}], uint32_t &pc, uint32_t mem, uint32_t &w0, uint32_t &w2, uint32_t &w3) {{")
         out.append(f"    {name}(A, X, S, pc, mem, w0, w2, w3);")
         out.append("  }")
