@@ -29,7 +29,6 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 # ptxas a control-flow graph of (#handlers x #opcodes) edges: its compile time explodes (> 30 min
 # for NX = 8).  With one shared dispatch point the graph has #handlers + #opcodes edges.
 THREADED = False
-PREFETCH = True
 THREADS = 128   # FX_THREADS: stride (in doubles) between spill slots of one thread
 
 
@@ -99,26 +98,21 @@ class Gen:
         self.lines.append(s)
 
     def dispatch(self):
-        """Fetch + decode + indirect branch.  With PREFETCH the instruction word of op i+1 is
-        loaded while op i is dispatched, so the shared-memory latency is off the per-op
-        dependency chain (mov -> shl -> ldc(table) -> brx -> handler)."""
-        if PREFETCH:
-            self.emit("mov.u32 c0, n0;")
-            self.emit("mov.b64 imm, {n2,n3};")
-            self.emit(f"ld.shared.v4.u32 {{n0,n1,n2,n3}}, [{self.pc}];")
-            self.emit(f"add.u32 {self.pc}, {self.pc}, 16;")
-            self.emit("and.b32 op, c0, 0xffff;")
-        else:
-            self.emit(f"ld.shared.v4.u32 {{c0,n1,n2,n3}}, [{self.pc}];")
-            self.emit(f"add.u32 {self.pc}, {self.pc}, 16;")
-            self.emit("and.b32 op, c0, 0xffff;")
-            self.emit("mov.b64 imm, {n2,n3};")
+        """Fetch + decode + indirect branch.  Split fetch: the opcode word of op i+1 is loaded one op
+        ahead (so decode -> table lookup -> BRX never waits on shared memory), the immediate of op i
+        is loaded at dispatch and arrives while the branch resolves.  No register copies: an
+        earlier version prefetched the whole 16-byte word and paid 8 MOVs per op for it."""
+        self.emit("and.b32 op, nop, 0xffff;")
+        self.emit(f"ld.shared.f64 imm, [{self.pc}+8];")
+        self.emit(f"ld.shared.u32 nop, [{self.pc}+16];")
+        self.emit(f"add.u32 {self.pc}, {self.pc}, 16;")
         self.emit("brx.idx op, TBL;")
 
     # ---- memory slots -----------------------------------------------------------------
     def mem_addr(self):
         """ma = mem + aux * (C*P*THREADS*8)"""
-        self.emit("shr.u32 ma, c0, 16;")
+        self.emit(f"ld.shared.u32 ma, [{self.pc}+-16];")
+        self.emit("shr.u32 ma, ma, 16;")
         self.emit(f"mad.lo.u32 ma, ma, {self.C * self.p * THREADS * 8}, {self.mem};")
 
     def mem_off(self, p, c):
@@ -320,22 +314,18 @@ class Gen:
                f"__device__ __forceinline__ void {name}({T} (&A)[{NL}][{self.p}], {T} (&X)[{self.nx}][{self.p}], "
                f"{T} (&S)[{NS}][{self.p}], uint32_t &pc, uint32_t mem, uint32_t &w0, uint32_t &w2, uint32_t &w3) {{",
                "  asm volatile(", '    "{\\n"',
-               '    ".reg .u32 c0, n0, n1, n2, n3, op, ma;\\n"', '    ".reg .f64 imm, zero, t0, t1, m0, m1;\\n"',
+               '    ".reg .u32 nop, op, ma;\\n"', '    ".reg .f64 imm, zero, t0, t1, m0, m1;\\n"',
                '    "mov.f64 zero, 0d0000000000000000;\\n"']
         tl = ", ".join(table)
         out.append(f'    "TBL: .branchtargets {tl};\\n"')
-        if PREFETCH:
-            self.emit(f"ld.shared.v4.u32 {{n0,n1,n2,n3}}, [{self.pc}];")
-            self.emit(f"add.u32 {self.pc}, {self.pc}, 16;")
+        self.emit(f"ld.shared.u32 nop, [{self.pc}];")
         self.emit("NEXT:")
         self.dispatch()
         for ln in self.lines + handlers:
             out.append(f'    "{ln}\\n"')
         out.append('    "EXIT:\\n"')
-        out.append(f'    "mov.u32 {self.w0}, c0;\\n"')
+        out.append(f'    "ld.shared.u32 {self.w0}, [{self.pc}+-16];\\n"')
         out.append(f'    "mov.b64 {{{self.w2},{self.w3}}}, imm;\\n"')
-        if PREFETCH:
-            out.append(f'    "sub.u32 {self.pc}, {self.pc}, 16;\\n"')
         out.append('    "}\\n"')
         outs = [o for o in self.operands if o[0][0] in "+="]
         ins = [o for o in self.operands if o[0][0] not in "+="]
