@@ -211,8 +211,11 @@ def run_b200(args):
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         pool = OraclePool()
         wl_s = make_workload(WORKLOAD, nsectors=2 * pool.cores)
-        pool.run(wl_s, pool.cores, 1 << 10)                      # warm
-        cpu = cpu_baseline(wl_s, pool, 2 * pool.cores, 1 << 14)
+        _, t_cal = pool.run(wl_s, 2 * pool.cores, 1 << 12)       # warm + calibrate: aim at ~15 s of CPU work
+        n_cpu = 1 << 12
+        while n_cpu < (1 << 21) and t_cal * (2 * n_cpu / (1 << 12)) < 20.0:
+            n_cpu *= 2
+        cpu = cpu_baseline(wl_s, pool, 2 * pool.cores, n_cpu)
         pool.close()
 
     # weak scaling: every rank integrates its own nsec_full sectors (distinct sector ids => distinct streams)
