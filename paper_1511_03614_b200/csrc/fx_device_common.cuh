@@ -52,10 +52,26 @@ struct fx_tpair {
   uint64_t e, o;
 };
 
-static __device__ __noinline__ fx_coord fx_lattice_coord(uint64_t t, const fx_transform *tf /* shared memory */) {
-  fx_coord c;
-  if (tf->r == 3) korobov_transform_r<3>(*tf, unit_from_t(t), c.x, c.xbar, c.w);  // the default weight: no switch
-  else korobov_transform(*tf, unit_from_t(t), c.x, c.xbar, c.w);
+// all P points of one coordinate per call: P independent dependency chains (int->double, Horner,
+// powers) overlap
+template <int P>
+struct fx_coordP {
+  double x[P], xbar[P], w[P];
+};
+template <int P>
+struct fx_tP {
+  uint64_t t[P];
+};
+template <int P>
+static __device__ __noinline__ fx_coordP<P> fx_lattice_coord(fx_tP<P> t, const fx_transform *tf /* shared memory */) {
+  fx_coordP<P> c;
+  if (tf->r == 3) {  // the default weight: no switch
+#pragma unroll
+    for (int p = 0; p < P; ++p) korobov_transform_r<3>(*tf, unit_from_t(t.t[p]), c.x[p], c.xbar[p], c.w[p]);
+  } else {
+#pragma unroll
+    for (int p = 0; p < P; ++p) korobov_transform(*tf, unit_from_t(t.t[p]), c.x[p], c.xbar[p], c.w[p]);
+  }
   return c;
 }
 
@@ -97,11 +113,13 @@ __device__ __forceinline__ void fx_make_points(const fx_integrate_params &prm, i
       if (k < dim) {
         // t_j = ((j g) mod 2^m) << (64-m) + Delta = j * (g << (64-m)) + Delta  (mod 2^64)
         const uint64_t G = prm.log2_n ? (prm.genvec[k] << (64 - prm.log2_n)) : 0ull;
+        fx_tP<P> tt;
+        FX_PLOOP { tt.t[p] = (j0 + p) * G + sh_delta[k]; }
+        const fx_coordP<P> c = fx_lattice_coord<P>(tt, tf);
         FX_PLOOP {
-          const fx_coord c = fx_lattice_coord((j0 + p) * G + sh_delta[k], tf);
-          x[k][p] = c.x;
-          xbar[k][p] = c.xbar;
-          W[p] *= c.w;
+          x[k][p] = c.x[p];
+          xbar[k][p] = c.xbar[p];
+          W[p] *= c.w[p];
         }
       } else {
         FX_PLOOP {

@@ -50,16 +50,40 @@ struct fx_fast;  // specialised by the generated file for the variants FX_WANT s
 #endif
 #include "fx_interp_gen.inc"
 
-// Library-backed operations, out of line: one copy each instead of P inlined copies per call site
-// (instruction-cache footprint, see fx_device_common.cuh).
-static __device__ __noinline__ double fx_slow_log(double a) { return t_log(a); }
-static __device__ __noinline__ double fx_slow_exp(double a) { return t_exp(a); }
-static __device__ __noinline__ cplx fx_slow_log(cplx a) { return t_log(a); }
-static __device__ __noinline__ cplx fx_slow_exp(cplx a) { return t_exp(a); }
-static __device__ __noinline__ cplx fx_slow_sqrt(cplx a) { return t_sqrt(a); }
-__device__ __forceinline__ double fx_slow_sqrt(double a) { return t_sqrt(a); }
-static __device__ __noinline__ cplx fx_slow_div(cplx a, cplx b) { return t_div(a, b); }
-__device__ __forceinline__ double fx_slow_div(double a, double b) { return t_div(a, b); }
+// Library-backed operations, out of line (one copy per kernel: instruction-cache footprint, see
+// fx_device_common.cuh) and over all P points of the thread at once, so that the P dependency
+// chains of a log or exp overlap instead of running one after the other.
+template <typename T, int P>
+struct fx_vec {
+  T v[P];
+};
+#define FX_SLOW_UNARY(name, fn)                                                  \
+  template <typename T, int P>                                                   \
+  static __device__ __noinline__ fx_vec<T, P> name(fx_vec<T, P> a) {             \
+    _Pragma("unroll") for (int p = 0; p < P; ++p) a.v[p] = fn(a.v[p]);           \
+    return a;                                                                    \
+  }
+FX_SLOW_UNARY(fx_slow_log, t_log)
+FX_SLOW_UNARY(fx_slow_exp, t_exp)
+FX_SLOW_UNARY(fx_slow_sqrt, t_sqrt)
+template <typename T, int P>
+static __device__ __noinline__ fx_vec<T, P> fx_slow_div(fx_vec<T, P> a, fx_vec<T, P> b) {
+#pragma unroll
+  for (int p = 0; p < P; ++p) a.v[p] = t_div(a.v[p], b.v[p]);
+  return a;
+}
+template <typename T, int P>
+__device__ __forceinline__ fx_vec<T, P> fx_pack(const T (&A)[P]) {
+  fx_vec<T, P> r;
+#pragma unroll
+  for (int p = 0; p < P; ++p) r.v[p] = A[p];
+  return r;
+}
+template <typename T, int P>
+__device__ __forceinline__ void fx_unpack(T (&A)[P], const fx_vec<T, P> &r) {
+#pragma unroll
+  for (int p = 0; p < P; ++p) A[p] = r.v[p];
+}
 
 // R[r] for a run-time r: only the slow path uses it (complex division by a register)
 template <typename T, int NX, int P>
@@ -94,27 +118,31 @@ __device__ __forceinline__ void fx_run(const fx_ins *prog, T (&X)[NX][P], const 
     if (op == FX_OUT) {
       sink(aux, A);
     } else if (op == FX_LOG) {
-      FX_PLOOP { A[p] = fx_slow_log(A[p]); }
+      fx_unpack(A, fx_slow_log(fx_pack<T, P>(A)));
     } else if (op == FX_EXP) {
-      FX_PLOOP { A[p] = fx_slow_exp(A[p]); }
+      fx_unpack(A, fx_slow_exp(fx_pack<T, P>(A)));
     } else if (op == FX_SQRT) {
-      FX_PLOOP { A[p] = fx_slow_sqrt(A[p]); }
+      fx_unpack(A, fx_slow_sqrt(fx_pack<T, P>(A)));
     } else if (op == FX_RDIVC) {
       FX_PLOOP { A[p] = t_rdivc(imm, A[p]); }
     } else if (op == FX_DIVM) {
-      FX_PLOOP { A[p] = fx_slow_div(A[p], M.ld(aux, p, P)); }
+      T R[P];
+      FX_PLOOP { R[p] = M.ld(aux, p, P); }
+      fx_unpack(A, fx_slow_div(fx_pack<T, P>(A), fx_pack<T, P>(R)));
     } else if (op == FX_RDIVM) {
-      FX_PLOOP { A[p] = fx_slow_div(M.ld(aux, p, P), A[p]); }
+      T R[P];
+      FX_PLOOP { R[p] = M.ld(aux, p, P); }
+      fx_unpack(A, fx_slow_div(fx_pack<T, P>(R), fx_pack<T, P>(A)));
     } else if (op >= FX_DIV_R && op < FX_DIV_R + FX_NR) {
       T R[P];
       FX_PLOOP { R[p] = A[p]; }
       fx_reg_dyn<T, NX, P>(op - FX_DIV_R, X, S, R);
-      FX_PLOOP { A[p] = fx_slow_div(A[p], R[p]); }
+      fx_unpack(A, fx_slow_div(fx_pack<T, P>(A), fx_pack<T, P>(R)));
     } else if (op >= FX_RDIV_R && op < FX_RDIV_R + FX_NR) {
       T R[P];
       FX_PLOOP { R[p] = A[p]; }
       fx_reg_dyn<T, NX, P>(op - FX_RDIV_R, X, S, R);
-      FX_PLOOP { A[p] = fx_slow_div(R[p], A[p]); }
+      fx_unpack(A, fx_slow_div(fx_pack<T, P>(R), fx_pack<T, P>(A)));
     } else {
       return;  // FX_END (or an opcode naming a variable this kernel does not have)
     }

@@ -106,7 +106,7 @@ class Gen:
         self.emit(f"ld.shared.f64 imm, [{self.pc}+8];")
         self.emit(f"ld.shared.u32 nop, [{self.pc}+16];")
         self.emit(f"add.u32 {self.pc}, {self.pc}, 16;")
-        self.emit("brx.idx op, TBL;")
+        self.emit("brx.idx.uni op, TBL;")
 
     # ---- memory slots -----------------------------------------------------------------
     def mem_addr(self):
