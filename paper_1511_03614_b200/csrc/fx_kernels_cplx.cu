@@ -39,15 +39,17 @@ __device__ __forceinline__ cplx det_lu(cplx (&J)[N][N]) {
     for (int r = c + 1; r < N; ++r) {
       const double mc = fma(J[c][c].re, J[c][c].re, J[c][c].im * J[c][c].im);
       const double mr = fma(J[r][c].re, J[r][c].re, J[r][c].im * J[r][c].im);
-      if (mr > mc) {
+      // row exchange by value selects (a branch around array element swaps keeps J in local memory)
+      const bool sw = mr > mc;
 #pragma unroll
-        for (int l = c; l < N; ++l) {
-          const cplx t = J[c][l];
-          J[c][l] = J[r][l];
-          J[r][l] = t;
-        }
-        det = t_neg(det);
+      for (int l = c; l < N; ++l) {
+        const cplx a = J[c][l], b = J[r][l];
+        J[c][l].re = sw ? b.re : a.re;
+        J[c][l].im = sw ? b.im : a.im;
+        J[r][l].re = sw ? a.re : b.re;
+        J[r][l].im = sw ? a.im : b.im;
       }
+      if (sw) det = t_neg(det);
     }
     const cplx piv = J[c][c];
     det = t_mul(det, piv);
@@ -100,12 +102,13 @@ __device__ __forceinline__ void fx_deform_points(const fx_ins *sh_deform, double
     const cplx d = det_lu(J);
 #pragma unroll
     for (int k = 0; k < N; ++k) M.st(k, p, P, zi[k]);
-    M.st(NGH, p, P, d.re);
-    M.st(NGH + (N > 1 ? 1 : N), p, P, d.im);
+    M.st(NGH + 2 * N, p, P, d.re);
+    M.st(NGH + 2 * N + 1, p, P, d.im);
   }
+  // x is re-read from its slot: nothing but J has to stay in registers across the elimination
 #pragma unroll
-  for (int k = 0; k < N; ++k) FX_PLOOP { X[k][p] = cplx{x[k][p], M.ld(k, p, P)}; }
-  FX_PLOOP { det[p] = cplx{M.ld(NGH, p, P), M.ld(NGH + (N > 1 ? 1 : N), p, P)}; }
+  for (int k = 0; k < N; ++k) FX_PLOOP { X[k][p] = cplx{M.ld(NGH + k, p, P), M.ld(k, p, P)}; }
+  FX_PLOOP { det[p] = cplx{M.ld(NGH + 2 * N, p, P), M.ld(NGH + 2 * N + 1, p, P)}; }
 }
 
 struct IntegrateSinkCplx {
