@@ -24,9 +24,9 @@
 #include <stdint.h>
 
 #define FX_NXMAX 12
-#define FX_NS 2
+#define FX_NS 1
 #define FX_NR (FX_NXMAX + FX_NS)
-#define FX_L 4  // accumulator levels
+#define FX_L 3  // accumulator levels
 #define FX_REG_S(j) (FX_NXMAX + (j))
 #define FX_LR (FX_L * FX_NR)  // opcodes of one (level, register) family
 
