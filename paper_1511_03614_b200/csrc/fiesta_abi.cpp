@@ -9,12 +9,14 @@
 #include <thread>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
 
 #include "../../include/fiesta_b200.h"
 #include "fx_compiler.hpp"
+#include "fx_jit.hpp"
 #include "fx_kernels.h"
 
 cudaError_t fx_launch_integrate_real(const fx_integrate_params &prm, cudaStream_t st);
@@ -72,6 +74,9 @@ struct fiesta_program {
   fx_ins *arena = nullptr;
   fx_sector_dev *sectors = nullptr;
   size_t arena_len = 0;
+  // native tier (fx_jit): one assembled kernel per real sector; function == nullptr -> interpreter
+  std::vector<fx::JitKernel> jit;
+  std::vector<std::string> jit_err;  // why a sector has no native kernel ("" if it has one or JIT is off)
 };
 
 namespace {
@@ -108,6 +113,9 @@ fx_transform_host make_transform(int r) {
 
 struct Plan {
   fx_integrate_params prm{};
+  const fiesta_program *pg = nullptr;
+  std::vector<int32_t> selv;  // selected sector indices (host copy)
+  bool native = false;        // every selected sector is real and has a native kernel, rule = lattice
   bool any_real = false, any_cplx = false;
   int Kmax = 0;
   size_t smem = 0;
@@ -182,6 +190,12 @@ int fiesta_compile(fiesta_ctx *ctx, const fiesta_sector_desc *sectors, int32_t n
   // sectors are independent: parse/optimise them on the host cores in parallel, then lay the
   // programs out in the arena in sector order
   std::vector<fx::CompiledSector> compiled(nsectors);
+  // FIESTA_JIT=0 keeps every sector on the interpreter (tests compare the two tiers)
+  const char *jit_env = std::getenv("FIESTA_JIT");
+  const bool jit_on = !(jit_env && jit_env[0] == '0');
+  std::vector<std::string> cubins(nsectors);
+  pg->jit.resize(nsectors);
+  pg->jit_err.assign(nsectors, "");
   {
     std::atomic<int> next{0};
     std::mutex err_mu;
@@ -197,6 +211,9 @@ int fiesta_compile(fiesta_ctx *ctx, const fiesta_sector_desc *sectors, int32_t n
             throw fx::CompileError{FIESTA_E_ARG, "n_orders must be in 1..8 and expr non-NULL"};
           compiled[s] = fx::compile_sector(d.expr, d.n_orders, dim, d.is_complex != 0, d.deform_f_index, d.lambda);
           compiled[s].sector_id = d.sector_id;
+          const fx::CompiledSector &cs = compiled[s];
+          if (jit_on && fx::jit_supported(cs.is_complex || cs.deform_on, dim))
+            if (!fx::jit_assemble(cs.main, dim, cs.K, cubins[s], pg->jit_err[s])) cubins[s].clear();
         } catch (fx::CompileError &e) {
           std::lock_guard<std::mutex> g(err_mu);
           if (s < err_sector) {
@@ -214,7 +231,7 @@ int fiesta_compile(fiesta_ctx *ctx, const fiesta_sector_desc *sectors, int32_t n
       }
     };
     unsigned nthr = std::min<unsigned>(std::max(1u, std::thread::hardware_concurrency()), 32u);
-    nthr = std::min<unsigned>(nthr, (unsigned)((nsectors + 7) / 8));
+    nthr = std::min<unsigned>(nthr, (unsigned)(jit_on ? nsectors : (nsectors + 7) / 8));
     if (nthr <= 1) {
       worker();
     } else {
@@ -266,6 +283,11 @@ int fiesta_compile(fiesta_ctx *ctx, const fiesta_sector_desc *sectors, int32_t n
     fiesta_program_free(pg);
     return cuda_fail(ctx, e, "program upload");
   }
+  {
+    const size_t smem = fx_integrate_smem_bytes_native(dim);
+    for (int s = 0; s < nsectors; ++s)
+      if (!cubins[s].empty() && !fx::jit_load(cubins[s], smem, pg->jit[s], pg->jit_err[s])) pg->jit[s] = fx::JitKernel{};
+  }
   *out = pg;
   return FIESTA_OK;
 }
@@ -275,6 +297,7 @@ void fiesta_program_free(fiesta_program *pg) {
   cudaSetDevice(pg->device);
   if (pg->arena) cudaFree(pg->arena);
   if (pg->sectors) cudaFree(pg->sectors);
+  for (fx::JitKernel &k : pg->jit) fx::jit_unload(k);
   delete pg;
 }
 

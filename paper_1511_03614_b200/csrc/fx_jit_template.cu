@@ -1,0 +1,93 @@
+// fx_jit_template.cu -- the evaluation kernel of real sectors with the program walk left OPEN.
+//
+// build.py compiles this file to PTX (one per NX), not to SASS.  The kernel is the same as
+// fx_integrate_real (points made on the device, periodising transform, accumulation, block-level
+// reduction: SURVEY 8(a) A1, A2, A6, A7) except that where the interpreter walks the instruction
+// program (A5, "a cycle through all the operations") it carries ONE marker line of
+// inline assembly naming the registers of x[k][p], W[p], the valid mask and the accumulator
+// address.  fiesta_compile (fx_jit.cpp) replaces that line, per sector, by the sector's fx_ins
+// program lowered to straight-line PTX on virtual registers -- the same operations in the same
+// order with the same roundings (.rn, explicit fma) as the interpreter's handlers -- and assembles
+// the result for sm_100a with the in-process PTX assembler.  The "internal form" of an integrand
+// is then native code: no fetch, no decode, no indirect branch, and ptxas does the register
+// allocation over all P points at once.
+//
+// Marker operand order (fx_jit.cpp parses it): nonfinite, valid, acc, W[0..P), x[0][0..P), x[1][..), ...
+#define FX_WANT(is_cplx, nx, p) 0  // no interpreter fast path in this translation unit
+#include "fx_device_common.cuh"
+
+#ifndef FXJ_NX
+#error "compile with -DFXJ_NX=4|8|12"
+#endif
+#ifndef FXJ_RULE
+#define FXJ_RULE FIESTA_RULE_LATTICE
+#endif
+
+// FP64 log/exp are library routines (CUDA math); the generated code calls these two
+extern "C" __device__ __noinline__ double fxj_log(double a) { return log(a); }
+extern "C" __device__ __noinline__ double fxj_exp(double a) { return exp(a); }
+
+#define FXJ_X4(k) "d"(x[k][0]), "d"(x[k][1]), "d"(x[k][2]), "d"(x[k][3])
+#if FXJ_NX == 4
+#define FXJ_FMT "%0 %1 %2 %3 %4 %5 %6 %7 %8 %9 %10 %11 %12 %13 %14 %15 %16 %17 %18 %19 %20 %21 %22"
+#define FXJ_XS FXJ_X4(0), FXJ_X4(1), FXJ_X4(2), FXJ_X4(3)
+#elif FXJ_NX == 8
+#define FXJ_FMT                                                                                              \
+  "%0 %1 %2 %3 %4 %5 %6 %7 %8 %9 %10 %11 %12 %13 %14 %15 %16 %17 %18 %19 %20 %21 %22 %23 %24 %25 %26 %27 " \
+  "%28 %29 %30 %31 %32 %33 %34 %35 %36 %37 %38"
+#define FXJ_XS FXJ_X4(0), FXJ_X4(1), FXJ_X4(2), FXJ_X4(3), FXJ_X4(4), FXJ_X4(5), FXJ_X4(6), FXJ_X4(7)
+#else
+#define FXJ_FMT                                                                                              \
+  "%0 %1 %2 %3 %4 %5 %6 %7 %8 %9 %10 %11 %12 %13 %14 %15 %16 %17 %18 %19 %20 %21 %22 %23 %24 %25 %26 %27 " \
+  "%28 %29 %30 %31 %32 %33 %34 %35 %36 %37 %38 %39 %40 %41 %42 %43 %44 %45 %46 %47 %48 %49 %50 %51 %52 %53 %54"
+#define FXJ_XS                                                                                             \
+  FXJ_X4(0), FXJ_X4(1), FXJ_X4(2), FXJ_X4(3), FXJ_X4(4), FXJ_X4(5), FXJ_X4(6), FXJ_X4(7), FXJ_X4(8), FXJ_X4(9), \
+      FXJ_X4(10), FXJ_X4(11)
+#endif
+
+extern "C" __global__ void __launch_bounds__(FX_THREADS, FXJ_NX <= 8 ? 4 : 2)
+    fxj_integrate(const __grid_constant__ fx_integrate_params prm) {
+  constexpr int P = FX_P_REAL;
+  constexpr int NX = FXJ_NX;
+  static_assert(P == 4, "the marker lists 4 points per variable");
+  extern __shared__ __align__(16) unsigned char smem[];
+  const int b = blockIdx.x;
+  const int chunk = b % prm.nchunks;
+  const int r = (b / prm.nchunks) % prm.n_shifts;
+  const int sel_idx = prm.sel_base + b / (prm.nchunks * prm.n_shifts);
+  const fx_sector_dev sec = prm.sectors[prm.sel[sel_idx]];
+  const int dim = prm.dim;
+  const fx_smem_layout L = fx_layout(0, 0, dim, prm.nbins, false);
+  double *sh_acc = reinterpret_cast<double *>(smem + L.acc);
+  uint64_t *sh_delta = reinterpret_cast<uint64_t *>(smem + L.delta);
+  double *sh_wsum = reinterpret_cast<double *>(smem + L.wsum);
+
+  fx_block_setup(prm, dim, (uint32_t)sec.sector_id, r, sel_idx, sh_delta, nullptr, nullptr);
+  const int nslots = 2 * sec.K;
+  for (int s = 0; s < nslots; ++s) sh_acc[s * FX_THREADS + threadIdx.x] = 0.0;
+  __syncthreads();
+
+  const uint64_t c0 = (uint64_t)chunk * prm.chunk;
+  const uint64_t c1 = min(c0 + prm.chunk, prm.n_per_shift);
+  unsigned nonfinite = 0;
+  const uint32_t acc = (uint32_t)__cvta_generic_to_shared(sh_acc + threadIdx.x);
+#pragma unroll 1
+  for (uint64_t base = c0 + (uint64_t)threadIdx.x * P; base < c1; base += (uint64_t)FX_THREADS * P) {
+    double x[NX][P], xbar[NX][P], W[P];
+    uint32_t bins[(NX + 3) / 4][P];
+    unsigned valid;
+    fx_make_points<FXJ_RULE, NX, P>(prm, dim, (uint32_t)sec.sector_id, sh_delta, nullptr, base, c1, x, xbar, W, valid, bins);
+    asm volatile("FXJIT_BODY " FXJ_FMT ";"
+                 : "+r"(nonfinite)
+                 : "r"(valid), "r"(acc), "d"(W[0]), "d"(W[1]), "d"(W[2]), "d"(W[3]), FXJ_XS
+                 : "memory");
+  }
+  if (prm.nsel < 0) {  // never true: keeps the two library wrappers in the PTX
+    sh_acc[threadIdx.x] = fxj_log(sh_acc[threadIdx.x]);
+    sh_acc[threadIdx.x + FX_THREADS] = fxj_exp(sh_acc[threadIdx.x + FX_THREADS]);
+  }
+  __syncthreads();
+  double *out = prm.partials + (((size_t)sel_idx * prm.n_shifts + r) * prm.nchunks + chunk) * FX_ACC_SLOTS;
+  fx_block_reduce(sh_acc, sh_wsum, nslots, out);
+  fx_block_finish(prm, dim, sel_idx, nonfinite, nullptr);
+}

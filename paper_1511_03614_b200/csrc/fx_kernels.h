@@ -55,6 +55,7 @@ struct fx_integrate_params {
   unsigned long long *nonfinite;  // [nsel]
   int32_t mem_doubles;       // shared-memory spill doubles per block (all threads)
   int32_t prog_ins_max;      // instructions reserved in shared memory (main + deform)
+  int32_t sel_base;          // native per-sector kernels (fx_jit): index into sel of the launch's first sector
 };
 
 struct fx_eval_params {
@@ -70,6 +71,7 @@ struct fx_eval_params {
 };
 
 size_t fx_integrate_smem_bytes(const fx_integrate_params &p);
+size_t fx_integrate_smem_bytes_native(int dim);  // native per-sector kernels: no program, no spill slots
 
 // S[nsel][R][FX_ACC_SLOTS] = sum over chunks of the partials, fixed order
 cudaError_t fx_launch_reduce_chunks(const double *partials, double *sums, int nsel, int R, int nchunks, cudaStream_t st);
