@@ -84,7 +84,16 @@ typedef struct {
   double flops;              /* FP64 flops per point counted as fma=2, mul/add=1, div=~15, log/exp~40 (nominal) */
 } fiesta_compile_info;
 
-/* Parse, optimise, register-allocate and upload.  `info` may be NULL, else [nsectors]. */
+/* Parse, optimise, register-allocate and upload.  `info` may be NULL, else [nsectors].
+ *
+ * Two forms of the same instruction program are produced ("transforms to an internal
+ * form"): (1) the fx_ins sequence, uploaded to the device arena and walked by the interpreter
+ * kernels (all rules, real and complex); (2) for real sectors, that same sequence lowered
+ * instruction by instruction to PTX, spliced into the evaluation kernel and assembled for sm_100a
+ * in process -- one native kernel per sector, used by fiesta_integrate / fiesta_partial_sums with
+ * the lattice rule when every selected sector has one.  Both forms perform the same operations in
+ * the same order with the same roundings: their sums are bit-identical.  The environment variable
+ * FIESTA_JIT=0 (read at each fiesta_compile) turns form (2) off. */
 int fiesta_compile(fiesta_ctx *ctx, const fiesta_sector_desc *sectors, int32_t nsectors, int32_t dim,
                    fiesta_program **out, fiesta_compile_info *info);
 void fiesta_program_free(fiesta_program *prog);
@@ -176,6 +185,10 @@ int fiesta_vegas_grid(fiesta_ctx *ctx, int32_t sector, int32_t dim, int32_t nbin
 /* Sum over sectors with errors combined in mean square.  Host arithmetic on
  * nsectors*K numbers; total_host[K]. */
 int fiesta_combine(const fiesta_result *per_sector_host, int32_t nsectors, int32_t K, fiesta_result *total_host);
+
+/* 1 if `sector` has a native kernel (form 2 above), else 0 with the reason in why_host (may be
+ * NULL; "" when the native tier is switched off or does not apply); <0 on bad arguments. */
+int fiesta_program_native(const fiesta_program *prog, int32_t sector, char *why_host, uint64_t buflen);
 
 /* Disassembly of a compiled sector (main program, then the deformation program) into buf. */
 int fiesta_program_dump(const fiesta_program *prog, int32_t sector, char *buf_host, uint64_t buflen);

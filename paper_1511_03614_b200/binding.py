@@ -62,6 +62,7 @@ _SIGNATURES = {
     "fiesta_vegas_grid": (C.c_int, [_VP, _I32, _I32, _I32, _VP, _VP]),
     "fiesta_combine": (C.c_int, [_VP, _I32, _I32, _VP]),
     "fiesta_program_dump": (C.c_int, [_VP, _I32, C.c_char_p, _U64]),
+    "fiesta_program_native": (C.c_int, [_VP, _I32, C.c_char_p, _U64]),
     "fiesta_fp64_peak": (C.c_int, [_VP, C.c_double, C.POINTER(C.c_double)]),
 }
 
@@ -133,6 +134,14 @@ class Program:
             self.handle = None
 
     __del__ = close
+
+    def native(self, sector=0):
+        """(has a native kernel, reason if not) -- fiesta_program_native"""
+        buf = C.create_string_buffer(4096)
+        rc = load_library().fiesta_program_native(self.handle, sector, buf, 4096)
+        if rc < 0:
+            raise FiestaError(rc, "fiesta_program_native")
+        return bool(rc), buf.value.decode()
 
     def dump(self, sector=0, buflen=1 << 20):
         buf = C.create_string_buffer(buflen)

@@ -61,6 +61,12 @@ struct fiesta_ctx {
   DevBuf<unsigned long long> nonfinite;
   DevBuf<fx_result_dev> results;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  // native per-sector kernels are spread over a few side streams, so that the blocks of the next
+  // sector's kernel fill the SMs while the last blocks of the previous one drain
+  static constexpr int NAUX = 4;
+  cudaStream_t aux[NAUX] = {};
+  cudaEvent_t aux_done[NAUX] = {};
+  cudaEvent_t fork = nullptr;
   bool timed = false;
   int n_launches = 0;
   int last_nsel = 0, last_dim = 0, last_nbins = 0;
@@ -148,7 +154,11 @@ int fiesta_create(fiesta_ctx **out, int cuda_device, void *cuda_stream) {
   c->stream = (cudaStream_t)cuda_stream;
   c->sm_count = prop.multiProcessorCount;
   c->smem_optin = prop.sharedMemPerBlockOptin;
-  if (cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess) {
+  bool aux_ok = cudaEventCreateWithFlags(&c->fork, cudaEventDisableTiming) == cudaSuccess;
+  for (int i = 0; i < fiesta_ctx::NAUX && aux_ok; ++i)
+    aux_ok = cudaStreamCreateWithFlags(&c->aux[i], cudaStreamNonBlocking) == cudaSuccess &&
+             cudaEventCreateWithFlags(&c->aux_done[i], cudaEventDisableTiming) == cudaSuccess;
+  if (!aux_ok || cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess) {
     delete c;
     return FIESTA_E_CUDA;
   }
@@ -171,6 +181,11 @@ void fiesta_destroy(fiesta_ctx *c) {
   c->scratch_u.release();
   c->nonfinite.release();
   c->results.release();
+  if (c->fork) cudaEventDestroy(c->fork);
+  for (int i = 0; i < fiesta_ctx::NAUX; ++i) {
+    if (c->aux_done[i]) cudaEventDestroy(c->aux_done[i]);
+    if (c->aux[i]) cudaStreamDestroy(c->aux[i]);
+  }
   if (c->ev0) cudaEventDestroy(c->ev0);
   if (c->ev1) cudaEventDestroy(c->ev1);
   delete c;
@@ -299,6 +314,12 @@ void fiesta_program_free(fiesta_program *pg) {
   if (pg->sectors) cudaFree(pg->sectors);
   for (fx::JitKernel &k : pg->jit) fx::jit_unload(k);
   delete pg;
+}
+
+int fiesta_program_native(const fiesta_program *pg, int32_t sector, char *why, uint64_t buflen) {
+  if (!pg || sector < 0 || sector >= (int)pg->host.size()) return FIESTA_E_ARG;
+  if (why && buflen) std::snprintf(why, buflen, "%s", pg->jit_err[sector].c_str());
+  return pg->jit[sector].function ? 1 : 0;
 }
 
 int fiesta_program_dump(const fiesta_program *pg, int32_t sector, char *buf, uint64_t buflen) {

@@ -71,8 +71,16 @@ extern "C" __global__ void __launch_bounds__(FX_THREADS, FXJ_NX <= 8 ? 4 : 2)
   const uint64_t c1 = min(c0 + prm.chunk, prm.n_per_shift);
   unsigned nonfinite = 0;
   const uint32_t acc = (uint32_t)__cvta_generic_to_shared(sh_acc + threadIdx.x);
+  // The trip count is the same for every thread of the block (points past the end are masked by
+  // `valid`), so the block can re-align its warps at every batch: a sector's native code is ~75 KB
+  // of straight-line instructions, far beyond the instruction caches, and warps that drift apart
+  // each stream it from L2 on their own; in step they share one stream.
 #pragma unroll 1
-  for (uint64_t base = c0 + (uint64_t)threadIdx.x * P; base < c1; base += (uint64_t)FX_THREADS * P) {
+  for (uint64_t it = c0; it < c1; it += (uint64_t)FX_THREADS * P) {
+    const uint64_t base = it + (uint64_t)threadIdx.x * P;
+    __syncthreads();
+    // out of line per coordinate, as in the interpreter kernels: inlining the NX x P transforms
+    // was measured slower (ptxas interleaves all of them: spills, twice the code)
     double x[NX][P], xbar[NX][P], W[P];
     uint32_t bins[(NX + 3) / 4][P];
     unsigned valid;

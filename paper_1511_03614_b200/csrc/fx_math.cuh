@@ -134,8 +134,12 @@ __device__ __forceinline__ void philox_t_pair(uint64_t seed, uint32_t sector_id,
 }
 
 // u = (2*(t>>12)+1) * 2^-53 in (0,1)   (R2)
+// Built from the bits instead of an int64 -> double conversion (a slow multi-instruction sequence on
+// the conversion pipe): with s = t>>12 < 2^52, d = 1 + s*2^-52 is the double with mantissa s;
+// d - 1 = s*2^-52 exactly, and adding 2^-53 gives (2s+1)*2^-53, which has 53 significant bits: exact.
 __device__ __forceinline__ double unit_from_t(uint64_t t) {
-  return (double)(long long)(2ull * (t >> 12) + 1ull) * 0x1p-53;
+  const double d = __longlong_as_double((long long)(0x3FF0000000000000ull | (t >> 12)));
+  return (d - 1.0) + 0x1p-53;
 }
 
 // lattice integer: (((j*g) mod N_L) << (64-m)) + delta, N_L = 2^m   (R2)

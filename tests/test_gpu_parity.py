@@ -161,6 +161,41 @@ def test_lattice_partial_sums_parity(fb, ctx, name, nsec, npts, nsh):
         assert np.all(res[si]["neval"] == wl.npoints) and np.all(res[si]["n_nonfinite"] == 0)
 
 
+@pytest.mark.parametrize("name,nsec,npts,nsh", [("C1", 1, 1 << 16, 8), ("C2", 3, 1 << 15, 1), ("C3", 2, 1 << 15, 8),
+                                                ("C5", 2, 1 << 13, 2), ("C3", 1, 64, 1), ("C2", 2, 8 * 256, 8)])
+def test_native_and_interpreter_tiers_agree_bitwise(fb, ctx, monkeypatch, name, nsec, npts, nsh):
+    """fiesta_compile's two forms of a real sector's program (interpreted fx_ins walk; the same
+    sequence assembled to a native kernel) do the same operations in the same order: every partial
+    sum and every result is bit-identical, and the interpreter tier on its own meets the oracle."""
+    wl = make_workload(name, nsectors=nsec, npoints=npts, n_shifts=nsh)
+    rule = fb.Rule(kind=fb.RULE_LATTICE, n_shifts=nsh, korobov_a=wl.korobov_a or 1129, periodize_r=3)
+    monkeypatch.setenv("FIESTA_JIT", "0")
+    prog_i = ctx.compile(wl.sectors, wl.dim)
+    monkeypatch.setenv("FIESTA_JIT", "1")
+    prog_n = ctx.compile(wl.sectors, wl.dim)
+    for si in range(nsec):
+        assert prog_i.native(si) == (False, "")
+        assert prog_n.native(si) == (True, ""), prog_n.native(si)
+    a = ctx.partial_sums(prog_i, npts, rule, wl.seed)
+    b = ctx.partial_sums(prog_n, npts, rule, wl.seed)
+    assert a.tobytes() == b.tobytes()
+    ra = ctx.integrate(prog_i, npts, rule, wl.seed)
+    rb = ctx.integrate(prog_n, npts, rule, wl.seed)
+    assert ra.tobytes() == rb.tobytes()
+    gv = OP.korobov_genvec(rule.korobov_a, npts // nsh, wl.dim)
+    s1, s2, sa = OI.lattice_partial_sums(spec(wl.sectors[0]), npts // nsh, nsh, gv, 3, wl.seed)
+    check_sums(a[0], s1, s2, sa)
+    # a selection that mixes the order, and a sector list of one
+    sel = list(range(nsec))[::-1]
+    assert ctx.partial_sums(prog_n, npts, rule, wl.seed, sectors=sel).tobytes() == a[sel].tobytes()
+
+
+def test_complex_sectors_stay_on_the_interpreter(fb, ctx):
+    wl = make_workload("C4", nsectors=1, npoints=1 << 12)
+    prog = ctx.compile(wl.sectors, wl.dim)
+    assert prog.native(0) == (False, "")
+
+
 def test_sector_selection_and_order(fb, ctx):
     """sectors=[2,0] integrates those two, in that order, with streams keyed by sector_id."""
     wl = make_workload("C2", nsectors=3, npoints=1 << 12)
