@@ -229,6 +229,7 @@ def run_b200(args):
     t_compile = time.perf_counter() - t0
     rule = fb.Rule.from_workload(wl)
     S = len(wl.sectors)
+    n_native = sum(1 for i in range(S) if prog.native(i)[0])     # sectors with an assembled native kernel
     evals_per_step = wl.evals                                    # points x sectors x orders, this rank
     flops_per_point = float(np.mean(prog.info["flops"]))         # nominal weights, DESIGN.md "Roofline"
     program_bytes = int(np.sum(prog.info["n_ir_ops"] + prog.info["n_deform_ops"] + 2)) * 16
@@ -299,14 +300,23 @@ def run_b200(args):
                        "naive_ops_per_point": wl.naive_ops_per_point, "ir_ops_per_point": float(np.mean(prog.info["n_ir_ops"])),
                        "l2": "flushed between iterations (256 MiB write); programs 16-32 MB, points made on device",
                        "parallelism": f"sectors sharded over {world} GPU(s), no data-path collective",
+                       "tier": ("native sm_100a kernel per sector (program lowered to PTX and assembled in fiesta_compile)"
+                                if n_native == S else "interpreter (fx_ins walk)"),
+                       "native_sectors": n_native,
                        "results_ok": ok, "generate_s": t_gen, "compile_s": t_compile},
             "gpu_launches": launches,
             "e2e": {"value": world * evals_per_step / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(sel.nbytes + 48),
                     "d2h_bytes_per_step": int(out.nbytes), "call": "fiesta_integrate (host sector list, host results)",
                     "compile_and_upload_s": t_compile, "program_bytes_uploaded_once": program_bytes},
             "roofline": {"bound": "alu", "achieved": ach, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                         "frac": ach / FP64_PEAK_TFLOPS, "traffic": None, "kernel": "fx_integrate_real<8>",
-                         "kernel_ms": kms, "flops_per_point": flops_per_point,
+                         "frac": ach / FP64_PEAK_TFLOPS,
+                         # dram__bytes_read+write of one native kernel launch (one sector, 2^24 points), ncu --set full,
+                         # profiles/r01_ncu_fxj_integrate.md; the algorithmic traffic is the 256-byte partial records
+                         "traffic": 372736 if n_native == S else None,
+                         "kernel": "fxj_integrate (one launch per sector)" if n_native == S else "fx_integrate_real<8>",
+                         "kernel_ms": kms, "kernel_launches_per_step": S if n_native == S else 1,
+                         "kernel_ms_per_launch": kms / (S if n_native == S else 1),
+                         "flops_per_point": flops_per_point,
                          "peak_source": "derived: 148 SM x 64 FP64 lanes x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP64 entry)",
                          "peak_dfma_microbench_live": peak_live},
             "clocks": clocks,
