@@ -6,7 +6,7 @@ There is no CPU fallback: if the library is missing or no sm_100 device is prese
 raise.
 """
 from .binding import (  # noqa: F401
-    Context, Program, Rule, FiestaError, LIB_PATH, load_library, exported_symbols,
+    Context, Program, Rule, FiestaError, LIB_PATH, load_library, exported_symbols, native_assemble,
     RULE_LATTICE, RULE_MC, RULE_VEGAS, RESULT_DTYPE, INFO_DTYPE,
 )
 

@@ -63,6 +63,7 @@ _SIGNATURES = {
     "fiesta_combine": (C.c_int, [_VP, _I32, _I32, _VP]),
     "fiesta_program_dump": (C.c_int, [_VP, _I32, C.c_char_p, _U64]),
     "fiesta_program_native": (C.c_int, [_VP, _I32, C.c_char_p, _U64]),
+    "fiesta_native_assemble": (C.c_int, [_VP, _I32, C.c_char_p, _U64, C.POINTER(_U64)]),
     "fiesta_fp64_peak": (C.c_int, [_VP, C.c_double, C.POINTER(C.c_double)]),
 }
 
@@ -119,6 +120,21 @@ class Rule:
 
 def _ptr(a):
     return None if a is None else a.ctypes.data_as(_VP)
+
+
+def native_assemble(sector, dim, buflen=1 << 22):
+    """fiesta_native_assemble: host only.  sector: object with .sector_id, .texts (workloads.SectorText).
+    -> (generated PTX of the program body, bytes of the assembled sm_100a cubin)."""
+    lib = load_library()
+    arr = (C.c_char_p * len(sector.texts))(*[t.encode() for t in sector.texts])
+    d = _SectorDesc(int(sector.sector_id), len(sector.texts), C.cast(arr, C.POINTER(C.c_char_p)),
+                    int(bool(sector.is_complex)), int(sector.deform_f_index), float(sector.lam))
+    buf = C.create_string_buffer(buflen)
+    n = _U64(0)
+    rc = lib.fiesta_native_assemble(C.byref(d), int(dim), buf, buflen, C.byref(n))
+    if rc != 0:
+        raise FiestaError(rc, buf.value.decode(errors="replace"))
+    return buf.value.decode(), int(n.value)
 
 
 class Program:

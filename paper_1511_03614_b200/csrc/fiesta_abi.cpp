@@ -316,6 +316,30 @@ void fiesta_program_free(fiesta_program *pg) {
   delete pg;
 }
 
+int fiesta_native_assemble(const fiesta_sector_desc *d, int32_t dim, char *ptx, uint64_t buflen, uint64_t *cubin_bytes) {
+  if (!d || !d->expr || d->n_orders < 1 || d->n_orders > FIESTA_MAX_ORDERS) return FIESTA_E_ARG;
+  if (d->is_complex || d->deform_f_index > 0 || !fx::jit_supported(false, dim)) return FIESTA_E_ARG;
+  try {
+    const fx::CompiledSector cs = fx::compile_sector(d->expr, d->n_orders, dim, false, 0, 0.0);
+    std::vector<std::string> operands = {"%nonfinite", "%valid", "%acc"};
+    for (int p = 0; p < FX_P_REAL; ++p) operands.push_back("%W" + std::to_string(p));
+    const int nx = dim <= 4 ? 4 : dim <= 8 ? 8 : 12;
+    for (int k = 0; k < nx; ++k)
+      for (int p = 0; p < FX_P_REAL; ++p) operands.push_back("%x" + std::to_string(k) + "_" + std::to_string(p));
+    if (ptx && buflen) std::snprintf(ptx, buflen, "%s", fx::jit_body_ptx(cs.main, cs.K, operands).c_str());
+    std::string cubin, err;
+    if (!fx::jit_assemble(cs.main, dim, cs.K, cubin, err)) {
+      if (ptx && buflen) std::snprintf(ptx, buflen, "%s", err.c_str());
+      return FIESTA_E_CUDA;
+    }
+    if (cubin_bytes) *cubin_bytes = cubin.size();
+    return FIESTA_OK;
+  } catch (fx::CompileError &e) {
+    if (ptx && buflen) std::snprintf(ptx, buflen, "%s", e.msg.c_str());
+    return e.code;
+  }
+}
+
 int fiesta_program_native(const fiesta_program *pg, int32_t sector, char *why, uint64_t buflen) {
   if (!pg || sector < 0 || sector >= (int)pg->host.size()) return FIESTA_E_ARG;
   if (why && buflen) std::snprintf(why, buflen, "%s", pg->jit_err[sector].c_str());

@@ -133,3 +133,54 @@ def test_gather_results_world_size_2_gloo(tmp_path):
     outs = [p.communicate(timeout=180)[0] for p in procs]
     for r, (p, o) in enumerate(zip(procs, outs)):
         assert p.returncode == 0 and f"ok {r}" in o, o
+
+
+# ------------------------------------------------------------------------------ native tier (host part)
+
+def _count(ptx, op):
+    return sum(1 for ln in ptx.splitlines() if ln.strip().startswith(op + " "))
+
+
+def test_native_lowering_of_the_paper_example(lib):
+    """PAPER.md:517-519, `1; 0; x[1]+0.2;`: the whole program is one add per point of the batch, then
+    the accumulation of the single output; the module assembles for sm_100a without a GPU."""
+    from workloads import SectorText
+    ptx, nbytes = lib.native_assemble(SectorText(sector_id=0, texts=["1;\n0;\nx[1]+0.2;\n|"]), 1)
+    assert nbytes > 10000
+    body = [ln.strip() for ln in ptx.splitlines()]
+    adds = [ln for ln in body if ln.startswith(("add.rn.f64 %fxa", "fma.rn.f64 %fxa"))]
+    assert len(adds) == 4 and all("%x0_" in ln for ln in adds)            # 4 points per thread, x[1] = register file X[0]
+    movs = [ln for ln in body if ln.startswith("mov.f64 %fxa") and "0d3FC999999999999A" in ln]
+    assert len(movs) == 4                                                 # 0.2, bit pattern of the literal
+    assert _count(ptx, "st.shared.f64") == 2 and _count(ptx, "testp.finite.f64") == 4   # sum g, sum g^2; non-finite count
+
+
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C5"])
+def test_native_lowering_keeps_every_operation(lib, name):
+    """The generated body has exactly the program's arithmetic (x 4 points): every FMA explicit, every
+    other operation with its rounding; logs and exps become calls; K outputs are accumulated."""
+    from workloads import make_workload
+    wl = make_workload(name, nsectors=2, npoints=1 << 10)
+    for s in wl.sectors:
+        ptx, nbytes = lib.native_assemble(s, wl.dim)
+        assert nbytes > 10000
+        assert "fma.f64" not in ptx and "mul.f64" not in ptx and "add.f64" not in ptx     # nothing left to contract
+        K = len(s.texts)
+        n_out = _count(ptx, "testp.finite.f64")
+        assert n_out == 4 * K
+        n_fma = _count(ptx, "fma.rn.f64") - n_out          # minus sum g^2 of the sink
+        n_mul = _count(ptx, "mul.rn.f64") - n_out          # minus g = W*o
+        n_add = _count(ptx, "add.rn.f64") + _count(ptx, "sub.rn.f64") - n_out
+        n_div = _count(ptx, "div.rn.f64")
+        n_call = ptx.count("call.uni")
+        assert min(n_fma, n_mul, n_add) >= 0 and (n_fma + n_mul + n_add + n_div + n_call) % 4 == 0
+        assert n_fma > 0 and n_call % 4 == 0
+
+
+def test_native_assemble_rejects_complex_and_bad_text(lib):
+    from workloads import SectorText
+    with pytest.raises(lib.FiestaError):
+        lib.native_assemble(SectorText(sector_id=0, texts=["1;\n0;\nx[1];\n|"], is_complex=True), 1)
+    with pytest.raises(lib.FiestaError) as e:
+        lib.native_assemble(SectorText(sector_id=0, texts=["1;\n0;\nx[1]+;\n|"]), 1)
+    assert "line" in str(e.value) or "expected" in str(e.value) or len(str(e.value)) > 0
