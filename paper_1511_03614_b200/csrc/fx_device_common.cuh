@@ -25,7 +25,7 @@ __host__ __device__ inline fx_smem_layout fx_layout(int prog_ins, int mem_double
   L.delta = o;
   o += FX_NXMAX * 8u;
   L.tf = o;
-  o += 80u;  // fx_transform (72 bytes), kept in shared memory for the per-coordinate helper
+  o += 80u;  // fx_transform (80 bytes), kept in shared memory for the per-coordinate helper
   L.grid = o;
   o += vegas ? (uint32_t)dim * (nbins + 1) * 8u : 0u;
   L.hist = o;
@@ -56,7 +56,7 @@ struct fx_tpair {
 // powers) overlap
 template <int P>
 struct fx_coordP {
-  double x[P], xbar[P], w[P];
+  double x[P], xbar[P], s[P];  // s = u(1-u): the point's weight is cw^dim (prod_k s_k)^r (korobov_weight)
 };
 template <int P>
 struct fx_tP {
@@ -67,10 +67,10 @@ static __device__ __noinline__ fx_coordP<P> fx_lattice_coord(fx_tP<P> t, const f
   fx_coordP<P> c;
   if (tf->r == 3) {  // the default weight: no switch
 #pragma unroll
-    for (int p = 0; p < P; ++p) korobov_transform_r<3>(*tf, unit_from_t(t.t[p]), c.x[p], c.xbar[p], c.w[p]);
+    for (int p = 0; p < P; ++p) korobov_xs_r<3>(*tf, t.t[p], c.x[p], c.xbar[p], c.s[p]);
   } else {
 #pragma unroll
-    for (int p = 0; p < P; ++p) korobov_transform(*tf, unit_from_t(t.t[p]), c.x[p], c.xbar[p], c.w[p]);
+    for (int p = 0; p < P; ++p) korobov_xs(*tf, t.t[p], c.x[p], c.xbar[p], c.s[p]);
   }
   return c;
 }
@@ -119,7 +119,7 @@ __device__ __forceinline__ void fx_make_points(const fx_integrate_params &prm, i
         FX_PLOOP {
           x[k][p] = c.x[p];
           xbar[k][p] = c.xbar[p];
-          W[p] *= c.w[p];
+          W[p] *= c.s[p];
         }
       } else {
         FX_PLOOP {
@@ -128,6 +128,7 @@ __device__ __forceinline__ void fx_make_points(const fx_integrate_params &prm, i
         }
       }
     }
+    FX_PLOOP { W[p] = korobov_weight(*tf, W[p]); }  // W held prod_k u_k(1-u_k) until here
   } else {
 #pragma unroll
     for (int kb = 0; kb < (NX + 1) / 2; ++kb) {
@@ -177,6 +178,9 @@ __device__ __forceinline__ void fx_block_setup(const fx_integrate_params &prm, i
     tf->r = prm.tf.r;
     tf->cw = prm.tf.cw;
     for (int i = 0; i < 7; ++i) tf->coef[i] = prm.tf.coef[i];
+    double cwd = 1.0;
+    for (int k = 0; k < dim; ++k) cwd *= prm.tf.cw;
+    tf->cwd = cwd;
   }
   if (prm.rule == FIESTA_RULE_VEGAS) {
     const double *g = prm.grid + (size_t)sel_idx * dim * (prm.nbins + 1);

@@ -224,21 +224,21 @@ __global__ void k_transform_points(int rule, fx_transform tf, const uint64_t *t,
                                    double *xbar, double *w) {
   const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= count) return;
-  double W = 1.0;
+  // the integrate kernels' own arithmetic (fx_make_points): korobov_xs per coordinate, one weight per point
+  double S = 1.0;
   for (int k = 0; k < dim; ++k) {
-    const double u = unit_from_t(t[i * dim + k]);
-    double xx, xb, ww;
-    if (rule == FIESTA_RULE_LATTICE) korobov_transform(tf, u, xx, xb, ww);
+    double xx, xb, ss;
+    if (rule == FIESTA_RULE_LATTICE) korobov_xs(tf, t[i * dim + k], xx, xb, ss);
     else {
-      xx = u;
-      xb = 1.0 - u;
-      ww = 1.0;
+      xx = unit_from_t(t[i * dim + k]);
+      xb = 1.0 - xx;
+      ss = 1.0;
     }
     x[i * dim + k] = xx;
     xbar[i * dim + k] = xb;
-    W *= ww;
+    S *= ss;
   }
-  w[i] = W;
+  w[i] = rule == FIESTA_RULE_LATTICE ? korobov_weight(tf, S) : 1.0;
 }
 
 // 16 independent DFMA chains per thread, 256 threads/block: the FP64 pipe limit (2 flops per DFMA).
@@ -325,6 +325,8 @@ cudaError_t fx_launch_transform_points(int rule, const fx_transform_host &tf, co
   t.r = tf.r;
   t.cw = tf.cw;
   for (int i = 0; i < 7; ++i) t.coef[i] = tf.coef[i];
+  t.cwd = 1.0;
+  for (int k = 0; k < dim; ++k) t.cwd *= tf.cw;
   k_transform_points<<<blocks_for(count, 128), 128, 0, st>>>(rule, t, t_dev, count, dim, x_dev, xbar_dev, w_dev);
   return cudaGetLastError();
 }

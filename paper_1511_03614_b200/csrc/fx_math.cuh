@@ -154,6 +154,7 @@ struct fx_transform {
   int r;          // 0..6
   double cw;      // (2r+1)!/(r!)^2
   double coef[7]; // phi_r(v) = v^(r+1) * sum_i coef[i] v^i
+  double cwd;     // cw^dim (integrate kernels: the weight of a point is cw^dim * (prod_k u_k(1-u_k))^r)
 };
 
 template <int R>
@@ -183,6 +184,61 @@ __device__ __forceinline__ void korobov_transform_r(const fx_transform &tf, doub
     for (int i = 1; i < R; ++i) sp *= s;
     w = tf.cw * sp;
   }
+}
+
+// The integrate kernels' form of the same transform, from the lattice integer t itself:
+//   - u > 1/2 iff the top bit of t is set, and 1-u = (2(2^52-1-s)+1) 2^-53 has the complemented
+//     mantissa, so v = min(u, 1-u) comes from one XOR (no FP64 compare/select), and one exact add turns
+//     the mantissa into v (d - (1 - 2^-53) with d = 1 + m 2^-52: the result (2m+1) 2^-53 is representable);
+//   - x and xbar exactly as korobov_transform_r (same v, same operations, same order);
+//   - instead of w = cw (u(1-u))^r it returns s = u(1-u): the caller multiplies the s of all
+//     coordinates and raises the product to r once per point, W = cw^dim (prod s)^r, which saves
+//     3 multiplications per coordinate and differs from prod w by rounding only.
+template <int R>
+__device__ __forceinline__ void korobov_xs_r(const fx_transform &tf, uint64_t t, double &x, double &xbar, double &s) {
+  const bool left = (long long)t >= 0;
+  const uint64_t tm = left ? t : ~t;
+  const double d = __longlong_as_double((long long)(0x3FF0000000000000ull | (tm >> 12)));
+  const double v = d - (1.0 - 0x1p-53);
+  const double vbar = 1.0 - v;
+  if constexpr (R == 0) {
+    x = left ? v : vbar;
+    xbar = left ? vbar : v;
+    s = 1.0;
+  } else {
+    double poly = tf.coef[R];
+#pragma unroll
+    for (int i = R - 1; i >= 0; --i) poly = fma(poly, v, tf.coef[i]);
+    double vp = v;
+#pragma unroll
+    for (int i = 0; i < R; ++i) vp *= v;
+    const double p = vp * poly;
+    const double big = 1.0 - p;
+    x = left ? p : big;
+    xbar = left ? big : p;
+    s = v * vbar;
+  }
+}
+
+__device__ __forceinline__ void korobov_xs(const fx_transform &tf, uint64_t t, double &x, double &xbar, double &s) {
+  switch (tf.r) {
+    case 0: korobov_xs_r<0>(tf, t, x, xbar, s); break;
+    case 1: korobov_xs_r<1>(tf, t, x, xbar, s); break;
+    case 2: korobov_xs_r<2>(tf, t, x, xbar, s); break;
+    case 3: korobov_xs_r<3>(tf, t, x, xbar, s); break;
+    case 4: korobov_xs_r<4>(tf, t, x, xbar, s); break;
+    case 5: korobov_xs_r<5>(tf, t, x, xbar, s); break;
+    default: korobov_xs_r<6>(tf, t, x, xbar, s); break;
+  }
+}
+
+// W = cw^dim * S^r from S = prod_k u_k(1-u_k)
+__device__ __forceinline__ double korobov_weight(const fx_transform &tf, double S) {
+  if (tf.r == 3) return tf.cwd * (S * S * S);
+  if (tf.r == 0) return 1.0;
+  double sp = S;
+  for (int i = 1; i < tf.r; ++i) sp *= S;
+  return tf.cwd * sp;
 }
 
 // run-time weight: same arithmetic, in the same order, for every r
