@@ -47,6 +47,8 @@ def parse_args():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--sectors", type=int, default=None, help="reduce the sector count (profiling runs only)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing (profiling runs only)")
+    ap.add_argument("--workload", default="C3", choices=["C1", "C2", "C3", "C4", "C5"],
+                    help="profiling runs only: time another BASELINE configuration (the bench line is C3)")
     return ap.parse_args()
 
 
@@ -207,7 +209,9 @@ def run_b200(args):
 
     # CPU oracle baseline first (rank 0, N=1 only), before this process touches CUDA heavily
     cpu = None
-    nsec_full = 2000 if args.sectors is None else args.sectors
+    global WORKLOAD
+    WORKLOAD = args.workload
+    nsec_full = args.sectors if args.sectors is not None else len(make_workload(WORKLOAD).sectors)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         pool = OraclePool()
         wl_s = make_workload(WORKLOAD, nsectors=2 * pool.cores)
@@ -293,9 +297,11 @@ def run_b200(args):
             "metric": METRIC, "value": world * evals_per_step * K / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world,
             "steps": K, "warmup": W, "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"BASELINE config 3 ({WORKLOAD}): {S} sectors/GPU, dim {wl.dim}, {wl.K} orders, "
-                                   f"{wl.npoints} points/sector = {wl.n_shifts} shifts x 2^{wl.n_lattice.bit_length() - 1} "
-                                   f"Korobov lattice (a={wl.korobov_a}), periodising r={wl.periodize_r}",
+            "config": {"workload": (f"BASELINE config 3 ({WORKLOAD}): {S} sectors/GPU, dim {wl.dim}, {wl.K} orders, "
+                                    f"{wl.npoints} points/sector = {wl.n_shifts} shifts x 2^{wl.n_lattice.bit_length() - 1} "
+                                    f"Korobov lattice (a={wl.korobov_a}), periodising r={wl.periodize_r}") if WORKLOAD == "C3" else
+                                   (f"PROFILING RUN, not the bench line: BASELINE config {WORKLOAD[1]}, {S} sectors/GPU, dim {wl.dim}, "
+                                    f"{wl.K} orders, {wl.npoints} points/sector, rule {wl.rule}"),
                        "sectors_per_gpu": S, "points_per_sector": wl.npoints, "orders": wl.K,
                        "naive_ops_per_point": wl.naive_ops_per_point, "ir_ops_per_point": float(np.mean(prog.info["n_ir_ops"])),
                        "l2": "flushed between iterations (256 MiB write); programs 16-32 MB, points made on device",
