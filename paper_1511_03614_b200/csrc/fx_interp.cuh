@@ -8,7 +8,7 @@
 //
 // Two levels:
 //   fast path  fx_fast<T,NX,P>::run  -- generated inline PTX (gen_interp_ptx.py): fetch, brx.idx
-//              dispatch and the arithmetic handlers, threaded code; runs until it meets an opcode
+//              dispatch and the arithmetic handlers; runs until it meets an opcode
 //              it does not implement and hands that instruction back;
 //   slow path  the switch below, in C++: outputs (FX_OUT), FX_END and the rare library-backed
 //              operations (log, exp; complex division, square root).  A few per point.

@@ -4,9 +4,12 @@
 Why PTX: nvcc lowers a C++ `switch` over ~400 opcodes to a compare-and-branch tree, and ptxas
 then re-copies the whole per-thread register state (X, S, A: 140+ registers) on every trip
 round the loop -- measured at ~600 cycles per interpreted op (profiles/r01_switch_baseline.md).
-Here the dispatch is one `brx.idx` through a `.branchtargets` table (SASS: BRX), every handler
-names its operand registers statically and ends with its own fetch + dispatch (threaded code),
-so the loop is: LDS.128 (fetch), LOP (decode), BRX, P x DFMA.
+Here the dispatch is one `brx.idx` through a `.branchtargets` table (SASS: LDC from the jump table,
+BRX), every handler names its operand registers statically and returns to the single dispatch
+point, so the loop is: LDS (opcode, prefetched), LDS.64 (immediate), decode, LDC, BRX, P x DFMA, BRA.
+Threaded code (a dispatch at the end of every handler) was measured twice and is slower on sm_100a
+(ptxas gives every brx.idx site its own constant-bank table, or, without the
+optimizer constant bank, its own island of BRA instructions).
 
 One function per (arithmetic type, NX variables, P points per thread):
 
