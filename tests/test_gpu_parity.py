@@ -525,8 +525,8 @@ def test_c2_full_size_sampled_sectors(fb, ctx):
 
 
 def test_c3_bench_configuration_sampled(fb, ctx):
-    """The workload bench.py times (config 3: dim 8, K = 5, 8 shifts x 2^21 points per sector,
-    16 chunks per (sector, shift)) on a slice of its sectors: one sampled (sector, shift) sum
+    """The workload bench.py times (config 3: dim 8, K = 5, 8 shifts x 2^21 points per sector, native
+    tier, two waves of blocks per sector) on a slice of its sectors: one sampled (sector, shift) sum
     against the oracle, and the properties that hold at any size -- per-shift sums agree with
     each other to the quoted error, results are finite, neval is exact."""
     wl = make_workload("C3", nsectors=6)
