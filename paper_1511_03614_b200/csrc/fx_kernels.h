@@ -9,7 +9,7 @@
 
 #define FX_THREADS 128   // threads per block of the evaluation kernels
 #define FX_P_REAL 4      // points per thread, real programs
-#define FX_P_CPLX 2      // points per thread, complex programs
+#define FX_P_CPLX 1      // points per thread, complex programs
 #define FX_ACC_SLOTS 32  // per-(sector,shift,chunk) partial record: [K<=8][C<=2][S1,S2]
 
 struct fx_sector_dev {       // one compiled sector in the device arena

@@ -9,7 +9,7 @@
 #ifndef FX_N
 #error "compile with -DFX_N=<dimension 1..8>"
 #endif
-#define FX_WANT(is_cplx, nx, p) ((nx) == FX_N && (p) == 2)  // real (deformation program) and complex, P = 2
+#define FX_WANT(is_cplx, nx, p) ((nx) == FX_N && (p) == 1)  // real (deformation program) and complex, P = 2
 #include "fx_device_common.cuh"
 
 #define FX_CAT2(a, b) a##b

@@ -350,8 +350,8 @@ class Gen:
 
 
 def main():
-    variants = [(False, nx, 4) for nx in (4, 8, 12)] + [(False, nx, 2) for nx in range(1, 9)] + \
-               [(True, nx, 2) for nx in range(1, 9)]
+    variants = [(False, nx, 4) for nx in (4, 8, 12)] + [(False, nx, 1) for nx in range(1, 9)] + \
+               [(True, nx, 1) for nx in range(1, 9)]
     print("// GENERATED by gen_interp_ptx.py -- do not edit.  See that file for the design.")
     for cplx, nx, p in variants:
         print(Gen(cplx, nx, p).function())
