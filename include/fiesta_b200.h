@@ -191,9 +191,9 @@ int fiesta_combine(const fiesta_result *per_sector_host, int32_t nsectors, int32
 int fiesta_program_native(const fiesta_program *prog, int32_t sector, char *why_host, uint64_t buflen);
 
 /* Host only (no context, no GPU): compile one real sector and run the native tier's lowering and
- * assembly on it.  Writes the generated PTX of the program body (NUL-terminated, truncated to
- * buflen) to ptx_body_host (may be NULL) and the size of the assembled sm_100a cubin to
- * cubin_bytes (may be NULL).  FIESTA_E_ARG for complex sectors; FIESTA_E_PARSE etc. as
+ * assembly on it.  Writes the generated PTX (the .const array of the program's FP64 immediates, then
+ * the program body; NUL-terminated, truncated to buflen) to ptx_body_host (may be NULL) and the
+ * size of the assembled sm_100a cubin to cubin_bytes (may be NULL).  FIESTA_E_ARG for complex sectors; FIESTA_E_PARSE etc. as
  * fiesta_compile; FIESTA_E_CUDA if the PTX assembler rejects the module (message in ptx_body_host). */
 int fiesta_native_assemble(const fiesta_sector_desc *sector, int32_t dim, char *ptx_body_host, uint64_t buflen,
                            uint64_t *cubin_bytes);

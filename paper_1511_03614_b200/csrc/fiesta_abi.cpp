@@ -322,11 +322,15 @@ int fiesta_native_assemble(const fiesta_sector_desc *d, int32_t dim, char *ptx, 
   try {
     const fx::CompiledSector cs = fx::compile_sector(d->expr, d->n_orders, dim, false, 0, 0.0);
     std::vector<std::string> operands = {"%nonfinite", "%valid", "%acc"};
-    for (int p = 0; p < FX_P_REAL; ++p) operands.push_back("%W" + std::to_string(p));
+    for (int p = 0; p < FXJ_P; ++p) operands.push_back("%W" + std::to_string(p));
     const int nx = dim <= 4 ? 4 : dim <= 8 ? 8 : 12;
     for (int k = 0; k < nx; ++k)
-      for (int p = 0; p < FX_P_REAL; ++p) operands.push_back("%x" + std::to_string(k) + "_" + std::to_string(p));
-    if (ptx && buflen) std::snprintf(ptx, buflen, "%s", fx::jit_body_ptx(cs.main, cs.K, operands).c_str());
+      for (int p = 0; p < FXJ_P; ++p) operands.push_back("%x" + std::to_string(k) + "_" + std::to_string(p));
+    if (ptx && buflen) {
+      std::string decl;
+      const std::string body = fx::jit_body_ptx(cs.main, cs.K, operands, &decl);
+      std::snprintf(ptx, buflen, "%s%s", decl.c_str(), body.c_str());  // the immediates' .const array, then the body
+    }
     std::string cubin, err;
     if (!fx::jit_assemble(cs.main, dim, cs.K, cubin, err)) {
       if (ptx && buflen) std::snprintf(ptx, buflen, "%s", err.c_str());

@@ -20,7 +20,8 @@ bool jit_supported(bool is_complex, int dim);
 bool jit_assemble(const std::vector<fx_ins> &prog, int dim, int K, std::string &cubin, std::string &err);
 
 // The PTX text of the program body alone (tests, disassembly).
-std::string jit_body_ptx(const std::vector<fx_ins> &prog, int K, const std::vector<std::string> &operands);
+std::string jit_body_ptx(const std::vector<fx_ins> &prog, int K, const std::vector<std::string> &operands,
+                         std::string *const_decl = nullptr);
 
 struct JitKernel {
   void *module = nullptr;    // CUmodule

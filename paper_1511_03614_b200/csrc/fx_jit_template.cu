@@ -27,29 +27,27 @@
 extern "C" __device__ __noinline__ double fxj_log(double a) { return log(a); }
 extern "C" __device__ __noinline__ double fxj_exp(double a) { return exp(a); }
 
-#define FXJ_X4(k) "d"(x[k][0]), "d"(x[k][1]), "d"(x[k][2]), "d"(x[k][3])
+#define FXJ_X2(k) "d"(x[k][0]), "d"(x[k][1])
 #if FXJ_NX == 4
-#define FXJ_FMT "%0 %1 %2 %3 %4 %5 %6 %7 %8 %9 %10 %11 %12 %13 %14 %15 %16 %17 %18 %19 %20 %21 %22"
-#define FXJ_XS FXJ_X4(0), FXJ_X4(1), FXJ_X4(2), FXJ_X4(3)
+#define FXJ_FMT "%0 %1 %2 %3 %4 %5 %6 %7 %8 %9 %10 %11 %12"
+#define FXJ_XS FXJ_X2(0), FXJ_X2(1), FXJ_X2(2), FXJ_X2(3)
 #elif FXJ_NX == 8
-#define FXJ_FMT                                                                                              \
-  "%0 %1 %2 %3 %4 %5 %6 %7 %8 %9 %10 %11 %12 %13 %14 %15 %16 %17 %18 %19 %20 %21 %22 %23 %24 %25 %26 %27 " \
-  "%28 %29 %30 %31 %32 %33 %34 %35 %36 %37 %38"
-#define FXJ_XS FXJ_X4(0), FXJ_X4(1), FXJ_X4(2), FXJ_X4(3), FXJ_X4(4), FXJ_X4(5), FXJ_X4(6), FXJ_X4(7)
+#define FXJ_FMT "%0 %1 %2 %3 %4 %5 %6 %7 %8 %9 %10 %11 %12 %13 %14 %15 %16 %17 %18 %19 %20"
+#define FXJ_XS FXJ_X2(0), FXJ_X2(1), FXJ_X2(2), FXJ_X2(3), FXJ_X2(4), FXJ_X2(5), FXJ_X2(6), FXJ_X2(7)
 #else
-#define FXJ_FMT                                                                                              \
-  "%0 %1 %2 %3 %4 %5 %6 %7 %8 %9 %10 %11 %12 %13 %14 %15 %16 %17 %18 %19 %20 %21 %22 %23 %24 %25 %26 %27 " \
-  "%28 %29 %30 %31 %32 %33 %34 %35 %36 %37 %38 %39 %40 %41 %42 %43 %44 %45 %46 %47 %48 %49 %50 %51 %52 %53 %54"
+#define FXJ_FMT \
+  "%0 %1 %2 %3 %4 %5 %6 %7 %8 %9 %10 %11 %12 %13 %14 %15 %16 %17 %18 %19 %20 %21 %22 %23 %24 %25 %26 %27 %28"
 #define FXJ_XS                                                                                             \
-  FXJ_X4(0), FXJ_X4(1), FXJ_X4(2), FXJ_X4(3), FXJ_X4(4), FXJ_X4(5), FXJ_X4(6), FXJ_X4(7), FXJ_X4(8), FXJ_X4(9), \
-      FXJ_X4(10), FXJ_X4(11)
+  FXJ_X2(0), FXJ_X2(1), FXJ_X2(2), FXJ_X2(3), FXJ_X2(4), FXJ_X2(5), FXJ_X2(6), FXJ_X2(7), FXJ_X2(8), FXJ_X2(9), \
+      FXJ_X2(10), FXJ_X2(11)
 #endif
 
-extern "C" __global__ void __launch_bounds__(FX_THREADS, FXJ_NX <= 8 ? 4 : 2)
+extern "C" __global__ void __launch_bounds__(FX_THREADS, FXJ_NX <= 8 ? 6 : 4)
     fxj_integrate(const __grid_constant__ fx_integrate_params prm) {
-  constexpr int P = FX_P_REAL;
+  constexpr int PB = FX_P_REAL;  // points per thread and batch: the interpreter's
+  constexpr int P = FXJ_P;       // points per pass of the program body
   constexpr int NX = FXJ_NX;
-  static_assert(P == 4, "the marker lists 4 points per variable");
+  static_assert(P == 2 && PB % P == 0, "the marker lists 2 points per variable");
   extern __shared__ __align__(16) unsigned char smem[];
   const int b = blockIdx.x;
   const int chunk = b % prm.nchunks;
@@ -57,7 +55,7 @@ extern "C" __global__ void __launch_bounds__(FX_THREADS, FXJ_NX <= 8 ? 4 : 2)
   const int sel_idx = prm.sel_base + b / (prm.nchunks * prm.n_shifts);
   const fx_sector_dev sec = prm.sectors[prm.sel[sel_idx]];
   const int dim = prm.dim;
-  const fx_smem_layout L = fx_layout(0, 0, dim, prm.nbins, false);
+  const fxj_smem_layout L = fxj_layout();
   double *sh_acc = reinterpret_cast<double *>(smem + L.acc);
   uint64_t *sh_delta = reinterpret_cast<uint64_t *>(smem + L.delta);
   double *sh_wsum = reinterpret_cast<double *>(smem + L.wsum);
@@ -76,19 +74,27 @@ extern "C" __global__ void __launch_bounds__(FX_THREADS, FXJ_NX <= 8 ? 4 : 2)
   // of straight-line instructions, far beyond the instruction caches, and warps that drift apart
   // each stream it from L2 on their own; in step they share one stream.
 #pragma unroll 1
-  for (uint64_t it = c0; it < c1; it += (uint64_t)FX_THREADS * P) {
-    const uint64_t base = it + (uint64_t)threadIdx.x * P;
-    __syncthreads();
-    // out of line per coordinate, as in the interpreter kernels: inlining the NX x P transforms
-    // was measured slower (ptxas interleaves all of them: spills, twice the code)
-    double x[NX][P], xbar[NX][P], W[P];
-    uint32_t bins[(NX + 3) / 4][P];
-    unsigned valid;
-    fx_make_points<FXJ_RULE, NX, P>(prm, dim, (uint32_t)sec.sector_id, sh_delta, nullptr, base, c1, x, xbar, W, valid, bins);
-    asm volatile("FXJIT_BODY " FXJ_FMT ";"
-                 : "+r"(nonfinite)
-                 : "r"(valid), "r"(acc), "d"(W[0]), "d"(W[1]), "d"(W[2]), "d"(W[3]), FXJ_XS
-                 : "memory");
+  for (uint64_t it = c0; it < c1; it += (uint64_t)FX_THREADS * PB) {
+    // A thread owns the same PB = 4 consecutive points per batch as in the interpreter kernel, but
+    // walks the program over them in two passes of P = 2.  With 4 points live (64 registers of x
+    // alone, 4 copies of every temporary) ptxas, held to 128 registers, serialises the points into
+    // dependent chains and over-subscribes the uniform registers the immediates live in; with 2 it
+    // interleaves both chains in 80 registers and 6 blocks are resident instead of 4.  Outputs are
+    // accumulated in point order either way, so the sums are unchanged (bit-identical to the
+    // interpreter's).
+#pragma unroll 1
+    for (int h = 0; h < PB / P; ++h) {
+      const uint64_t base = it + (uint64_t)threadIdx.x * PB + (uint64_t)h * P;
+      __syncthreads();
+      double x[NX][P], xbar[NX][P], W[P];
+      uint32_t bins[(NX + 3) / 4][P];
+      unsigned valid;
+      fx_make_points<FXJ_RULE, NX, P>(prm, dim, (uint32_t)sec.sector_id, sh_delta, nullptr, base, c1, x, xbar, W, valid, bins);
+      asm volatile("FXJIT_BODY " FXJ_FMT ";"
+                   : "+r"(nonfinite)
+                   : "r"(valid), "r"(acc), "d"(W[0]), "d"(W[1]), FXJ_XS
+                   : "memory");
+    }
   }
   if (prm.nsel < 0) {  // never true: keeps the two library wrappers in the PTX
     sh_acc[threadIdx.x] = fxj_log(sh_acc[threadIdx.x]);

@@ -73,6 +73,24 @@ struct fx_eval_params {
 size_t fx_integrate_smem_bytes(const fx_integrate_params &p);
 size_t fx_integrate_smem_bytes_native(int dim);  // native per-sector kernels: no program, no spill slots
 
+// Shared-memory layout of the native kernels (fx_jit_template.cu): accumulators for K <= 8 real
+// outputs (sum g, sum g^2: 16 slots, one column per thread), the lattice shifts, the transform
+// parameters (fx_block_setup puts them right after the shifts), the block reduction's per-warp sums.
+#define FXJ_ACC_SLOTS 16
+#define FXJ_P 2  // points per thread and pass of the native program body (two passes per batch of FX_P_REAL)
+struct fxj_smem_layout {
+  uint32_t acc, delta, tf, wsum, total;
+};
+static inline __host__ __device__ fxj_smem_layout fxj_layout() {
+  fxj_smem_layout L;
+  L.acc = 0;
+  L.delta = FXJ_ACC_SLOTS * FX_THREADS * 8u;
+  L.tf = L.delta + FX_NXMAX * 8u;
+  L.wsum = L.tf + 80u;
+  L.total = L.wsum + FXJ_ACC_SLOTS * (FX_THREADS / 32) * 8u;
+  return L;
+}
+
 // S[nsel][R][FX_ACC_SLOTS] = sum over chunks of the partials, fixed order
 cudaError_t fx_launch_reduce_chunks(const double *partials, double *sums, int nsel, int R, int nchunks, cudaStream_t st);
 

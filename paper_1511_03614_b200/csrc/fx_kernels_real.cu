@@ -135,7 +135,7 @@ size_t fx_integrate_smem_bytes(const fx_integrate_params &prm) {
   return fx_layout(prm.prog_ins_max, prm.mem_doubles, prm.dim, prm.nbins, prm.rule == FIESTA_RULE_VEGAS).total;
 }
 
-size_t fx_integrate_smem_bytes_native(int dim) { return fx_layout(0, 0, dim, 1, false).total; }
+size_t fx_integrate_smem_bytes_native(int) { return fxj_layout().total; }
 
 cudaError_t fx_launch_integrate_real(const fx_integrate_params &prm, cudaStream_t st) {
   const size_t smem = fx_integrate_smem_bytes(prm);
