@@ -70,7 +70,7 @@ extern "C" __global__ void __launch_bounds__(FX_THREADS, FXJ_NX <= 8 ? 6 : 4)
   unsigned nonfinite = 0;
   const uint32_t acc = (uint32_t)__cvta_generic_to_shared(sh_acc + threadIdx.x);
   // The trip count is the same for every thread of the block (points past the end are masked by
-  // `valid`), so the block can re-align its warps at every batch: a sector's native code is ~75 KB
+  // `valid`), so the block can re-align its warps at every pass: a sector's native code is ~45 KB
   // of straight-line instructions, far beyond the instruction caches, and warps that drift apart
   // each stream it from L2 on their own; in step they share one stream.
 #pragma unroll 1
