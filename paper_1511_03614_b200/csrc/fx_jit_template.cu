@@ -27,6 +27,55 @@
 extern "C" __device__ __noinline__ double fxj_log(double a) { return log(a); }
 extern "C" __device__ __noinline__ double fxj_exp(double a) { return exp(a); }
 
+struct fxj_xs {
+  double x, s;
+};
+// weights other than the default r = 3: one out-of-line copy
+static __device__ __noinline__ fxj_xs fxj_transform_any(const fx_transform *tf, uint64_t t) {
+  fxj_xs c;
+  double xb;
+  korobov_xs(*tf, t, c.x, xb, c.s);
+  return c;
+}
+
+// Lattice points of one pass, inline (2 points x NX coordinates; with 4 points live inlining was slower) and
+// without xbar = 1-x, which real programs never read.  Same arithmetic and order as
+// fx_make_points<FIESTA_RULE_LATTICE>: x and W are bit-identical.
+template <int NX, int P>
+__device__ __forceinline__ void fxj_make_points(const fx_integrate_params &prm, int dim, const uint64_t *sh_delta,
+                                                uint64_t j0, uint64_t jend, double (&x)[NX][P], double (&W)[P],
+                                                unsigned &valid) {
+  valid = 0;
+  FX_PLOOP {
+    W[p] = 1.0;
+    if (j0 + p < jend) valid |= 1u << p;
+  }
+  const fx_transform *tf = reinterpret_cast<const fx_transform *>(sh_delta + FX_NXMAX);
+  const bool r3 = tf->r == 3;
+#pragma unroll
+  for (int k = 0; k < NX; ++k) {
+    if (k < dim) {
+      const uint64_t G = prm.log2_n ? (prm.genvec[k] << (64 - prm.log2_n)) : 0ull;
+      const uint64_t d = sh_delta[k];
+      FX_PLOOP {
+        const uint64_t t = (j0 + p) * G + d;
+        double xb, sv;
+        if (r3) {
+          korobov_xs_r<3>(*tf, t, x[k][p], xb, sv);
+        } else {
+          const fxj_xs c = fxj_transform_any(tf, t);
+          x[k][p] = c.x;
+          sv = c.s;
+        }
+        W[p] *= sv;
+      }
+    } else {
+      FX_PLOOP { x[k][p] = 0.5; }
+    }
+  }
+  FX_PLOOP { W[p] = korobov_weight(*tf, W[p]); }
+}
+
 #define FXJ_X2(k) "d"(x[k][0]), "d"(x[k][1])
 #if FXJ_NX == 4
 #define FXJ_FMT "%0 %1 %2 %3 %4 %5 %6 %7 %8 %9 %10 %11 %12"
@@ -86,10 +135,9 @@ extern "C" __global__ void __launch_bounds__(FX_THREADS, FXJ_NX <= 8 ? 6 : 4)
     for (int h = 0; h < PB / P; ++h) {
       const uint64_t base = it + (uint64_t)threadIdx.x * PB + (uint64_t)h * P;
       __syncthreads();
-      double x[NX][P], xbar[NX][P], W[P];
-      uint32_t bins[(NX + 3) / 4][P];
+      double x[NX][P], W[P];
       unsigned valid;
-      fx_make_points<FXJ_RULE, NX, P>(prm, dim, (uint32_t)sec.sector_id, sh_delta, nullptr, base, c1, x, xbar, W, valid, bins);
+      fxj_make_points<NX, P>(prm, dim, sh_delta, base, c1, x, W, valid);
       asm volatile("FXJIT_BODY " FXJ_FMT ";"
                    : "+r"(nonfinite)
                    : "r"(valid), "r"(acc), "d"(W[0]), "d"(W[1]), FXJ_XS
