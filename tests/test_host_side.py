@@ -153,7 +153,7 @@ def test_native_lowering_of_the_paper_example(lib):
     assert body[0].startswith(".const .align 8 .f64 fxj_const[1] = {0d3FC999999999999A}")   # 0.2, bit pattern
     movs = [ln for ln in body if ln.startswith("mov.f64 %fxa") and ln.endswith("%fxc;")]
     assert len(movs) == 2 and "ld.const.f64 %fxc, [fxj_const+0];" in body
-    assert _count(ptx, "st.shared.f64") == 2 and _count(ptx, "testp.finite.f64") == 2   # sum g, sum g^2; non-finite count
+    assert _count(ptx, "st.shared.f64") == 2 and _count(ptx, "setp.eq.u32 %fxf,") == 2   # sum g, sum g^2; non-finite count
 
 
 @pytest.mark.parametrize("name", ["C1", "C2", "C3", "C5"])
@@ -167,7 +167,7 @@ def test_native_lowering_keeps_every_operation(lib, name):
         assert nbytes > 10000
         assert "fma.f64" not in ptx and "mul.f64" not in ptx and "add.f64" not in ptx     # nothing left to contract
         K = len(s.texts)
-        n_out = _count(ptx, "testp.finite.f64")
+        n_out = _count(ptx, "setp.eq.u32 %fxf,")
         assert n_out == 2 * K
         n_fma = _count(ptx, "fma.rn.f64") - n_out          # minus sum g^2 of the sink
         n_mul = _count(ptx, "mul.rn.f64") - n_out          # minus g = W*o
