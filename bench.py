@@ -318,7 +318,7 @@ def run_b200(args):
                          "frac": ach / FP64_PEAK_TFLOPS,
                          # dram__bytes_read+write of one native kernel launch (one sector, 2^24 points), ncu --set full,
                          # profiles/r01_ncu_fxj_integrate.md; the algorithmic traffic is the 256-byte partial records
-                         "traffic": 510976 if n_native == S else None,
+                         "traffic": 55296 if n_native == S else None,
                          "kernel": "fxj_integrate (one launch per sector)" if n_native == S else "fx_integrate_real<8>",
                          "kernel_ms": kms, "kernel_launches_per_step": S if n_native == S else 1,
                          "kernel_ms_per_launch": kms / (S if n_native == S else 1),
