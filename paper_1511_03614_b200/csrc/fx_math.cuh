@@ -157,43 +157,14 @@ struct fx_transform {
   double cwd;     // cw^dim (integrate kernels: the weight of a point is cw^dim * (prod_k u_k(1-u_k))^r)
 };
 
-template <int R>
-__device__ __forceinline__ void korobov_transform_r(const fx_transform &tf, double u, double &x, double &xbar,
-                                                    double &w) {
-  const double ubar = 1.0 - u;  // exact: u is an odd multiple of 2^-53
-  if constexpr (R == 0) {
-    x = u;
-    xbar = ubar;
-    w = 1.0;
-  } else {
-    const double v = fmin(u, ubar);
-    double poly = tf.coef[R];
-#pragma unroll
-    for (int i = R - 1; i >= 0; --i) poly = fma(poly, v, tf.coef[i]);
-    double vp = v;
-#pragma unroll
-    for (int i = 0; i < R; ++i) vp *= v;
-    const double p = vp * poly;
-    const double big = 1.0 - p;
-    const bool left = u <= ubar;
-    x = left ? p : big;
-    xbar = left ? big : p;
-    const double s = u * ubar;
-    double sp = s;
-#pragma unroll
-    for (int i = 1; i < R; ++i) sp *= s;
-    w = tf.cw * sp;
-  }
-}
-
-// The integrate kernels' form of the same transform, from the lattice integer t itself:
+// From the lattice integer t itself:
 //   - u > 1/2 iff the top bit of t is set, and 1-u = (2(2^52-1-s)+1) 2^-53 has the complemented
 //     mantissa, so v = min(u, 1-u) comes from one XOR (no FP64 compare/select), and one exact add turns
 //     the mantissa into v (d - (1 - 2^-53) with d = 1 + m 2^-52: the result (2m+1) 2^-53 is representable);
-//   - x and xbar exactly as korobov_transform_r (same v, same operations, same order);
+//   - x = phi_r(u) and xbar = 1 - x both from v, whichever side u is on (R4: full relative accuracy at both faces);
 //   - instead of w = cw (u(1-u))^r it returns s = u(1-u): the caller multiplies the s of all
 //     coordinates and raises the product to r once per point, W = cw^dim (prod s)^r, which saves
-//     3 multiplications per coordinate and differs from prod w by rounding only.
+//     3 multiplications per coordinate and differs from prod w by rounding only (R4).
 template <int R>
 __device__ __forceinline__ void korobov_xs_r(const fx_transform &tf, uint64_t t, double &x, double &xbar, double &s) {
   const bool left = (long long)t >= 0;
@@ -245,20 +216,6 @@ __device__ __forceinline__ double korobov_weight(const fx_transform &tf, double 
   double sp = S;
   for (int i = 1; i < tf.r; ++i) sp *= S;
   return tf.cwd * sp;
-}
-
-// run-time weight: same arithmetic, in the same order, for every r
-__device__ __forceinline__ void korobov_transform(const fx_transform &tf, double u, double &x, double &xbar,
-                                                  double &w) {
-  switch (tf.r) {
-    case 0: korobov_transform_r<0>(tf, u, x, xbar, w); break;
-    case 1: korobov_transform_r<1>(tf, u, x, xbar, w); break;
-    case 2: korobov_transform_r<2>(tf, u, x, xbar, w); break;
-    case 3: korobov_transform_r<3>(tf, u, x, xbar, w); break;
-    case 4: korobov_transform_r<4>(tf, u, x, xbar, w); break;
-    case 5: korobov_transform_r<5>(tf, u, x, xbar, w); break;
-    default: korobov_transform_r<6>(tf, u, x, xbar, w); break;
-  }
 }
 
 // Vegas map of one coordinate (R8): exact integer bin and fraction, then the edges.
