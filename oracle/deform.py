@@ -158,6 +158,22 @@ def gradient_and_hessian(prog: Program, f_index: int, x, dtype=LD):
     return g, h
 
 
+def permanent(a):
+    """per a[j,:,:] = sum over permutations of prod_k a[j,k,perm(k)]: the Leibniz formula of the
+    determinant with every sign +.  For a matrix of magnitudes it is the magnitude companion (R14) of
+    det; n! terms, n <= 8."""
+    import itertools
+    a = np.asarray(a)
+    npts, n, _ = a.shape
+    out = np.zeros(npts, dtype=a.dtype)
+    for perm in itertools.permutations(range(n)):
+        term = np.ones(npts, dtype=a.dtype)
+        for k in range(n):
+            term = term * a[:, k, perm[k]]
+        out = out + term
+    return out
+
+
 def deform(prog: Program, f_index: int, lam, x, xbar=None, rdtype=LD):
     """(z, J) for real points x[j,:]; xbar = 1-x may be passed if known more accurately (R4)."""
     cdtype = CLD if rdtype == LD else np.complex128

@@ -144,14 +144,22 @@ def evaluate(prog: Program, x, dtype=LD):
 class _MagWalker(_Walker):
     """Walks (value, magnitude) pairs.  DESIGN.md R14.
 
-    M is a first-order bound on how far rounding of the leaves and of every
-    operation can move the value, in units of the rounding unit:
-      leaf: |v|;  a+-b: Ma+Mb;  a*b: Ma*Mb;  a/b: Ma*Mb/|b|^2;
-      integer power: via the product rule;  e^q: |e^q| * max(1,|q|*Me/|e|);
-      log e: max(|log e|,1) + Me/|e|.
-    For sign-definite inputs (all leaves and coefficients positive, no
-    subtraction) M equals |f| except through the real-power rule (factor |q|)
-    and the log rule.
+    M >= |v| is the scale a per-point "relative 1e-12" has to be measured against when the
+    expression cancels.  For sums it is R14's modulus tree; through products, quotients, powers and
+    logarithms the EXCESS M - |v| (the part of M that comes from cancellation below) is carried to
+    first order, the way relative rounding errors propagate:
+      leaf:     |v|
+      a +- b:   Ma + Mb                                    (R14: "every subtraction by addition")
+      a * b:    |ab| (1 + ra + rb)  = Ma|b| + |a|Mb - |ab|         with r = M/|v| - 1
+      a / b:    |a/b| (1 + ra + rb)
+      e^n:      |e^n| (1 + |n| re)       (n integer; n < 0 as the reciprocal of e^|n|)
+      e^q:      |e^q| (1 + |q| re)       d(e^q)/e^q = q de/e
+      log e:    max(|log e|, 1) + re     d(log e) = de/e;  R14's clamp of |log| at 1
+    Where nothing cancels (r = 0 at every node: C1, C2, C5, and C3 except through the logarithm
+    polynomials) M = |f| up to the clamp, and the test is the plain relative one.  R14's literal
+    wording (modulus tree through * and / too) multiplies the factors (1 + r) instead of adding the
+    r: never smaller than this M, and for quotients and negative powers of a cancelling argument it
+    is not even a bound; DESIGN.md section 3 lists this reading.
     """
 
     def fm(self, i):
@@ -176,35 +184,40 @@ class _MagWalker(_Walker):
         if op == "mul":
             a, ma = self.walk(node[1])
             b, mb = self.walk(node[2])
-            return a * b, ma * mb
+            aa, ab = np.abs(a), np.abs(b)
+            return a * b, ma * ab + aa * mb - aa * ab
         if op == "div":
             a, ma = self.walk(node[1])
             b, mb = self.walk(node[2])
-            return a / b, ma * mb / (np.abs(b) ** 2)
+            aa, ab = np.abs(a), np.abs(b)
+            return a / b, ma / ab + aa * mb / (ab * ab) - aa / ab
         if op == "pow":
             e, me = self.walk(node[1])
             q = node[2]
+            ae = np.abs(e)
             if float(q).is_integer():
                 qi = int(q)
                 v = _int_power(e, qi)
-                m = _int_power(me, abs(qi))
-                if qi < 0:
-                    m = m / np.abs(_int_power(e, abs(qi))) ** 2
-                return v, m
+                if qi == 0:
+                    return v, np.abs(v)
+                n = abs(qi)
+                w = np.abs(_int_power(e, n))
+                mw = w + n * np.abs(_int_power(e, n - 1)) * (me - ae)   # |e|^n + n|e|^(n-1)(Me-|e|)
+                return v, (mw if qi > 0 else mw / (w * w))
             if self.cplx:
                 v = np.exp(self.rdt.type(q) * np.log(e))
             else:
                 v = np.power(e, self.rdt.type(q))
-            return v, np.abs(v) * np.maximum(1, abs(q) * me / np.abs(e))
+            return v, np.abs(v) * (1 + abs(q) * (me / ae - 1))
         if op == "log":
             e, me = self.walk(node[1])
             v = np.log(e)
-            return v, np.maximum(np.abs(v), 1) + me / np.abs(e)
+            return v, np.maximum(np.abs(v), 1) + (me / np.abs(e) - 1)
         raise ValueError(op)
 
 
 def evaluate_with_magnitude(prog: Program, x, dtype=LD):
-    """(f(x_j), M(x_j)) with M the magnitude companion of DESIGN.md R14."""
+    """(f(x_j), M(x_j)) with M the magnitude companion of DESIGN.md R14 (see _MagWalker)."""
     x = np.asarray(x, dtype=dtype)
     with np.errstate(all="ignore"):
         v, m = _MagWalker(prog, x, dtype).walk(prog.final)

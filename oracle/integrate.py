@@ -42,7 +42,7 @@ class SectorSpec:
 
 
 def neumaier_sum(values):
-    """Compensated sum of a 1-D long-double array in index order (O6)."""
+    """Compensated sum of a 1-D long-double array in index order (kept for small arrays)."""
     s = values.dtype.type(0)
     c = values.dtype.type(0)
     for v in values:
@@ -53,6 +53,71 @@ def neumaier_sum(values):
             c += (v - t) + s
         s = t
     return s + c
+
+
+_BIAS = 16600  # long double exponents lie in (-16446, 16385): value = integer * 2^-(_BIAS+64)
+
+
+class ExactSum:
+    """O6: sum_j v_j as the plain definition -- the EXACT sum of the terms, rounded once at the end.
+
+    Every finite long double is an integer times a power of two, v = M * 2^(e-64) with
+    |M| < 2^64 (np.frexp).  The integers M are added without rounding (numpy int64 per
+    exponent value, then Python integers), so the order of the terms, and how a caller feeds
+    them in pieces, cannot change the result.  NaN / Inf terms make the sum NaN / Inf.
+    """
+
+    def __init__(self):
+        self.total = 0          # exact sum = total * 2^-(_BIAS+64)
+        self.special = LD(0)    # plain sum of the non-finite terms (propagates NaN / Inf)
+        self.has_special = False
+
+    def add(self, values):
+        v = np.asarray(values, dtype=LD).ravel()
+        fin = np.isfinite(v)
+        if not np.all(fin):
+            self.special = self.special + np.sum(v[~fin])
+            self.has_special = True
+            v = v[fin]
+        for i in range(0, v.shape[0], 1 << 20):
+            self._add_finite(v[i:i + (1 << 20)])
+        return self
+
+    def _add_finite(self, v):
+        if v.shape[0] == 0:
+            return
+        m, e = np.frexp(v)                       # v = m * 2^e, 0.5 <= |m| < 1 (or m = 0)
+        a = np.abs(m) * LD(2.0 ** 32)
+        hi = np.floor(a)                         # top 32 bits of the 64-bit integer mantissa
+        lo = (a - hi) * LD(2.0 ** 32)            # low 32 bits; both conversions are exact
+        sign = np.where(m < 0, -1.0, 1.0)
+        e0 = int(e.min())
+        idx = (e - e0).astype(np.int64)
+        # per exponent, sums of at most 2^20 integers < 2^32: exact in float64
+        shi = np.bincount(idx, weights=hi.astype(np.float64) * sign)
+        slo = np.bincount(idx, weights=lo.astype(np.float64) * sign)
+        for k in np.nonzero((shi != 0) | (slo != 0))[0]:
+            part = (int(shi[k]) << 32) + int(slo[k])
+            self.total += part << (int(k) + e0 + _BIAS)
+
+    def value(self):
+        if self.has_special:
+            return self.special
+        n = abs(self.total)
+        if n == 0:
+            return LD(0)
+        shift = max(n.bit_length() - 64, 0)
+        q, rem = n >> shift, n & ((1 << shift) - 1)
+        if shift and (rem > (1 << (shift - 1)) or (rem == (1 << (shift - 1)) and (q & 1))):
+            q += 1                               # round to nearest, ties to even
+        x = LD(float(q >> 32)) * LD(2.0 ** 32) + LD(float(q & 0xFFFFFFFF))   # halves < 2^33: exact
+        x = np.ldexp(x, shift - _BIAS - 64)
+        return -x if self.total < 0 else x
+
+
+def exact_sum(values):
+    """Exact sum of an array of long doubles, rounded once (see ExactSum)."""
+    return ExactSum().add(values).value()
 
 
 def integrand_values(sec: SectorSpec, x, xbar=None, rdtype=LD):
@@ -89,34 +154,37 @@ def lattice_points(sec: SectorSpec, n_lattice, genvec, r_periodize, seed, shift_
 
 
 def lattice_partial_sums(sec: SectorSpec, n_lattice, n_shifts, genvec, r_periodize, seed, chunk=1 << 14, rdtype=LD,
-                         shifts=None):
+                         shifts=None, first=0, count=None):
     """S1[r,k,c] = sum_j g, S2[r,k,c] = sum_j g^2, SA[r,k,c] = sum_j |g|, g = W*o_k component c.
 
-    Shapes [R, K, C], C = 1 (real) or 2 (Re, Im).  Sums run in index order over j (O6).
-    `shifts`: optional subset of shift indices to compute (the other rows stay 0); used to
-    sample single shifts of a full-size run.
+    Shapes [R, K, C], C = 1 (real) or 2 (Re, Im).  Each sum is the exact sum of its terms rounded
+    once (O6, ExactSum); `chunk` only bounds the memory of one evaluation and cannot change a result.
+    `shifts`: optional subset of shift indices to compute (the other rows stay 0); `first`, `count`:
+    optional sub-range j = first..first+count-1 of the lattice; both are used to sample pieces of a
+    full-size run.
     """
     ncomp = 2 if (sec.is_complex or sec.deform_f_index > 0) else 1
     s1 = np.zeros((n_shifts, sec.K, ncomp), dtype=rdtype)
     s2 = np.zeros_like(s1)
     sa = np.zeros_like(s1)
+    last = n_lattice if count is None else first + count
     for r in (range(n_shifts) if shifts is None else shifts):
-        parts = [[[[], [], []] for _ in range(ncomp)] for _ in range(sec.K)]
-        for first in range(0, n_lattice, chunk):
-            cnt = min(chunk, n_lattice - first)
-            x, xbar, w = lattice_points(sec, n_lattice, genvec, r_periodize, seed, r, first, cnt, rdtype)
+        acc = [[[ExactSum(), ExactSum(), ExactSum()] for _ in range(ncomp)] for _ in range(sec.K)]
+        for f0 in range(first, last, chunk):
+            cnt = min(chunk, last - f0)
+            x, xbar, w = lattice_points(sec, n_lattice, genvec, r_periodize, seed, r, f0, cnt, rdtype)
             vals = integrand_values(sec, x, xbar, rdtype)
             for k in range(sec.K):
                 for c, comp in enumerate(_components(vals[k])):
                     g = w * comp
-                    parts[k][c][0].append(np.sum(g))
-                    parts[k][c][1].append(np.sum(g * g))
-                    parts[k][c][2].append(np.sum(np.abs(g)))
+                    acc[k][c][0].add(g)
+                    acc[k][c][1].add(g * g)
+                    acc[k][c][2].add(np.abs(g))
         for k in range(sec.K):
             for c in range(ncomp):
-                s1[r, k, c] = neumaier_sum(np.array(parts[k][c][0], dtype=rdtype))
-                s2[r, k, c] = neumaier_sum(np.array(parts[k][c][1], dtype=rdtype))
-                sa[r, k, c] = neumaier_sum(np.array(parts[k][c][2], dtype=rdtype))
+                s1[r, k, c] = acc[k][c][0].value()
+                s2[r, k, c] = acc[k][c][1].value()
+                sa[r, k, c] = acc[k][c][2].value()
     return s1, s2, sa
 
 
@@ -154,21 +222,28 @@ def mc_points(sec: SectorSpec, seed, iteration, first, count, rdtype=LD):
     return t, P.unit_from_t(t, rdtype)
 
 
-def integrate_mc(sec: SectorSpec, npoints, seed, chunk=1 << 14, rdtype=LD):
-    """Plain Monte Carlo: x = u, W = 1; value, sigma per (order, component) (R5)."""
+def mc_partial_sums(sec: SectorSpec, npoints, seed, iteration=0, chunk=1 << 14, rdtype=LD, first=0, count=None):
+    """Plain MC (x = u, W = 1): S1[k,c] = sum_j o_k, S2[k,c] = sum_j o_k^2 over points first..first+count-1
+    of the Philox MC stream (default: all npoints); exact sums rounded once (O6)."""
     ncomp = 2 if (sec.is_complex or sec.deform_f_index > 0) else 1
-    p1 = [[[] for _ in range(ncomp)] for _ in range(sec.K)]
-    p2 = [[[] for _ in range(ncomp)] for _ in range(sec.K)]
-    for first in range(0, npoints, chunk):
-        cnt = min(chunk, npoints - first)
-        _, y = mc_points(sec, seed, 0, first, cnt, rdtype)
+    acc = [[[ExactSum(), ExactSum()] for _ in range(ncomp)] for _ in range(sec.K)]
+    last = npoints if count is None else first + count
+    for f0 in range(first, last, chunk):
+        cnt = min(chunk, last - f0)
+        _, y = mc_points(sec, seed, iteration, f0, cnt, rdtype)
         vals = integrand_values(sec, y, None, rdtype)
         for k in range(sec.K):
             for c, comp in enumerate(_components(vals[k])):
-                p1[k][c].append(np.sum(comp))
-                p2[k][c].append(np.sum(comp * comp))
-    s1 = np.array([[neumaier_sum(np.array(p1[k][c], dtype=rdtype)) for c in range(ncomp)] for k in range(sec.K)], dtype=rdtype)
-    s2 = np.array([[neumaier_sum(np.array(p2[k][c], dtype=rdtype)) for c in range(ncomp)] for k in range(sec.K)], dtype=rdtype)
+                acc[k][c][0].add(comp)
+                acc[k][c][1].add(comp * comp)
+    s1 = np.array([[acc[k][c][0].value() for c in range(ncomp)] for k in range(sec.K)], dtype=rdtype)
+    s2 = np.array([[acc[k][c][1].value() for c in range(ncomp)] for k in range(sec.K)], dtype=rdtype)
+    return s1, s2
+
+
+def integrate_mc(sec: SectorSpec, npoints, seed, chunk=1 << 14, rdtype=LD):
+    """Plain Monte Carlo: x = u, W = 1; value, sigma per (order, component) (R5)."""
+    s1, s2 = mc_partial_sums(sec, npoints, seed, 0, chunk, rdtype)
     return estimate_from_sums(s1[None], s2[None], npoints)
 
 
@@ -238,12 +313,14 @@ def vegas_refine(grid_d, hist_d, alpha):
 
 
 def vegas_iteration_sums(sec: SectorSpec, grid, npoints, seed, iteration, chunk=1 << 14, rdtype=LD):
-    """S1[K,C], S2[K,C] and histogram h[dim, NB] (sum over orders/components of g^2) of one iteration."""
+    """S1[K,C], S2[K,C] and histogram h[dim, NB] (sum over orders/components of g^2) of one iteration.
+
+    All three are exact sums of their terms rounded once (O6, ExactSum): the histogram bin h[d][b]
+    is the sum of g^2 over the points whose coordinate d falls in bin b."""
     ncomp = 2 if (sec.is_complex or sec.deform_f_index > 0) else 1
     nbins = grid.shape[1] - 1
-    p1 = [[[] for _ in range(ncomp)] for _ in range(sec.K)]
-    p2 = [[[] for _ in range(ncomp)] for _ in range(sec.K)]
-    hist = np.zeros((sec.dim, nbins), dtype=rdtype)
+    acc = [[[ExactSum(), ExactSum()] for _ in range(ncomp)] for _ in range(sec.K)]
+    hacc = [[ExactSum() for _ in range(nbins)] for _ in range(sec.dim)]
     for first in range(0, npoints, chunk):
         cnt = min(chunk, npoints - first)
         t, _ = mc_points(sec, seed, iteration, first, cnt, rdtype)
@@ -253,13 +330,19 @@ def vegas_iteration_sums(sec: SectorSpec, grid, npoints, seed, iteration, chunk=
         for k in range(sec.K):
             for c, comp in enumerate(_components(vals[k])):
                 g = w * comp
-                p1[k][c].append(np.sum(g))
-                p2[k][c].append(np.sum(g * g))
+                acc[k][c][0].add(g)
+                acc[k][c][1].add(g * g)
                 g2 = g2 + g * g
         for d in range(sec.dim):
-            np.add.at(hist[d], b[:, d], g2)      # h[d][b] += g^2, one point after another
-    s1 = np.array([[neumaier_sum(np.array(p1[k][c], dtype=rdtype)) for c in range(ncomp)] for k in range(sec.K)], dtype=rdtype)
-    s2 = np.array([[neumaier_sum(np.array(p2[k][c], dtype=rdtype)) for c in range(ncomp)] for k in range(sec.K)], dtype=rdtype)
+            order = np.argsort(b[:, d], kind="stable")
+            bs, gs = b[order, d], g2[order]
+            cuts = np.searchsorted(bs, np.arange(nbins + 1))
+            for bb in range(nbins):
+                if cuts[bb + 1] > cuts[bb]:
+                    hacc[d][bb].add(gs[cuts[bb]:cuts[bb + 1]])
+    s1 = np.array([[acc[k][c][0].value() for c in range(ncomp)] for k in range(sec.K)], dtype=rdtype)
+    s2 = np.array([[acc[k][c][1].value() for c in range(ncomp)] for k in range(sec.K)], dtype=rdtype)
+    hist = np.array([[hacc[d][bb].value() for bb in range(nbins)] for d in range(sec.dim)], dtype=rdtype)
     return s1, s2, hist
 
 

@@ -98,7 +98,7 @@ def test_mc_transform_is_identity(fb, ctx):
 
 # ------------------------------------------------------------------------------ A5: program walk
 
-def _eval_case(ctx, wl, nsec, npts, seed):
+def _eval_case(ctx, wl, nsec, npts, seed, label=None):
     prog = ctx.compile(wl.sectors, wl.dim)
     rng = np.random.default_rng(seed)
     x = rng.random((npts, wl.dim))
@@ -111,7 +111,7 @@ def _eval_case(ctx, wl, nsec, npts, seed):
     for si in range(nsec):
         got = ctx.eval_points(prog, si, x)
         ref, mag = oracle_values_and_magnitude(spec(wl.sectors[si]), x)
-        worst = max(worst, check_points(got, ref, mag))
+        worst = max(worst, check_points(got, ref, mag, label=None if label is None else f"{label} sector {si}"))
     prog.close()
     return worst
 
@@ -120,7 +120,7 @@ def _eval_case(ctx, wl, nsec, npts, seed):
                                             ("C5", 4, 999)])
 def test_per_point_parity_configs(ctx, name, nsec, npts):
     wl = make_workload(name, nsectors=nsec, npoints=1 << 12)
-    assert _eval_case(ctx, wl, nsec, npts, 11) <= 1.0
+    assert _eval_case(ctx, wl, nsec, npts, 11, label=f"per-point {name}") <= 1.0
 
 
 @pytest.mark.parametrize("npts", [1, 3, 511, 512, 513])

@@ -17,7 +17,7 @@ from oracle.deform import (deform, det_lu, differentiate, evaluate_deformed, f_p
 from oracle.evaluate import CLD, LD, evaluate, evaluate_with_magnitude, polygamma_const, PI, EULER_GAMMA
 from oracle.integrate import (SectorSpec, combine_sectors, estimate_from_sums, integrate_lattice, integrate_mc,
                               integrate_vegas, lattice_partial_sums, neumaier_sum, vegas_combine, vegas_refine,
-                              vegas_uniform_grid)
+                              vegas_uniform_grid, exact_sum, ExactSum, mc_partial_sums, vegas_iteration_sums)
 from oracle.parser import ParseError, parse
 from workloads import korobov_a
 
@@ -425,6 +425,59 @@ def test_c4_workload_has_negative_imaginary_f():
 
 # ------------------------------------------------------------------ estimators
 
+def test_exact_sum_against_rationals():
+    """O6: the oracle's sums are the exact sum of the terms rounded once.  Pin: Python Fractions (every
+    long double is a dyadic rational), math.fsum on doubles, cancelling cases, any feeding order."""
+    from fractions import Fraction
+
+    def frac(v):                      # exact value of a long double: mantissa (two exact halves) * 2^e
+        m, e = np.frexp(LD(v))
+        a = abs(m) * LD(2.0 ** 32)
+        hi = int(np.floor(a))
+        lo = int((a - LD(hi)) * LD(2.0 ** 32))
+        q = Fraction((hi << 32) + lo) * Fraction(2) ** (int(e) - 64)
+        return -q if m < 0 else q
+
+    rng = np.random.default_rng(7)
+    for trial in range(20):
+        n = int(rng.integers(1, 400))
+        v = (rng.standard_normal(n).astype(LD) * LD(3) + rng.standard_normal(n).astype(LD) * LD(2.0 ** -60)) \
+            * LD(2.0) ** rng.integers(-200, 200, n).astype(LD)
+        if trial % 3 == 0:            # heavy cancellation: the big terms vanish exactly
+            v = np.concatenate([v, -v, rng.standard_normal(5).astype(LD) * LD(2.0 ** -300)])
+            v = v[rng.permutation(v.shape[0])]
+        exact = sum((frac(x) for x in v), Fraction(0))
+        got = exact_sum(v)
+        # rounded once: within half an ulp (2^-64 relative) of the rational sum, or exactly 0
+        assert exact == 0 and got == 0 or abs(frac(got) - exact) <= abs(exact) * Fraction(1, 2 ** 64)
+        acc = ExactSum()              # fed in pieces, reversed: the same number
+        for piece in np.array_split(v[::-1], 7):
+            acc.add(piece)
+        assert acc.value() == got
+    d = rng.standard_normal(5000) * 10.0 ** rng.integers(-10, 10, 5000)
+    assert float(exact_sum(d.astype(LD))) == math.fsum(d)
+    assert exact_sum(np.array([LD(1), LD(2) ** -70, -LD(1), LD(2) ** -70], dtype=LD)) == LD(2) ** -69
+    assert np.isnan(exact_sum(np.array([LD(1), LD(np.nan)], dtype=LD)))
+    assert exact_sum(np.zeros(0, dtype=LD)) == 0
+
+
+def test_sums_do_not_depend_on_chunking():
+    """The chunk argument of the oracle's integrators only bounds memory."""
+    sec = SectorSpec([block(2, ["1+x[1]*x[2]"], "p[f[1],-2]*l[f[1]]-0.3*x[1]")], sector_id=3)
+    a = lattice_partial_sums(sec, 1 << 10, 2, [1, 333], 3, SEED, chunk=1 << 14)
+    b = lattice_partial_sums(sec, 1 << 10, 2, [1, 333], 3, SEED, chunk=37)
+    assert all(np.array_equal(x, y) for x, y in zip(a, b))
+    whole = lattice_partial_sums(sec, 1 << 10, 2, [1, 333], 3, SEED, shifts=[1])
+    left = lattice_partial_sums(sec, 1 << 10, 2, [1, 333], 3, SEED, shifts=[1], first=0, count=300)
+    right = lattice_partial_sums(sec, 1 << 10, 2, [1, 333], 3, SEED, shifts=[1], first=300, count=724)
+    assert np.allclose((left[0] + right[0]).astype(float), whole[0].astype(float), rtol=1e-17)
+    assert all(np.array_equal(x, y) for x, y in zip(mc_partial_sums(sec, 1000, 5, chunk=1000), mc_partial_sums(sec, 1000, 5, chunk=64)))
+    grid = vegas_uniform_grid(2, 7)
+    a = vegas_iteration_sums(sec, grid, 999, 5, 2, chunk=999)
+    b = vegas_iteration_sums(sec, grid, 999, 5, 2, chunk=100)
+    assert all(np.array_equal(x, y) for x, y in zip(a, b))
+
+
 def test_neumaier_and_estimators():
     v = np.array([LD(1), LD(2) ** -70, -LD(1), LD(2) ** -70], dtype=LD)
     assert neumaier_sum(v) == LD(2) ** -69
@@ -553,3 +606,92 @@ def test_magnitude_companion_bounds_the_value():
     prog = parse(block(1, [], "(x[1]+1)-(x[1]+0.9999)"))
     v, m = evaluate_with_magnitude(prog, x[:, :1])
     assert np.all(m / np.abs(v) > 1e4)
+
+
+def test_magnitude_companion_rules_on_hand_numbers():
+    """The first-order rules of oracle/evaluate.py::_MagWalker on numbers worked by hand (DESIGN.md R14)."""
+    x = np.array([[0.25]], dtype=LD)
+    # a = 1 - x = 0.75 with Ma = 1.25 (ra = 2/3);  b = x + 2 = 2.25, Mb = 2.25 (rb = 0)
+    a, ma = 0.75, 1.25
+    cases = {
+        "(1-x[1])*(x[1]+2)": a * 2.25 * (1 + 2 / 3),
+        "(1-x[1])/(x[1]+2)": a / 2.25 * (1 + 2 / 3),
+        "(x[1]+2)/(1-x[1])": 2.25 / a * (1 + 2 / 3),
+        "p[1-x[1],3]": a ** 3 * (1 + 3 * 2 / 3),
+        "p[1-x[1],-2]": a ** -2 * (1 + 2 * 2 / 3),
+        "p[1-x[1],-2.5]": a ** -2.5 * (1 + 2.5 * 2 / 3),
+        "l[1-x[1]]": 1 + 2 / 3,                                   # |log 0.75| < 1: the clamp
+        "l[p[1-x[1],20]]": abs(20 * math.log(0.75)) + 20 * 2 / 3,
+        "(1-x[1])*(1-x[1])*(1-x[1])": a ** 3 * (1 + 3 * 2 / 3),   # products add the excesses
+        "(1-x[1])-(x[1]+2)": ma + 2.25,
+    }
+    for text, want in cases.items():
+        v, m = evaluate_with_magnitude(parse(block(1, [], text)), x)
+        assert abs(float(m[0]) - want) < 1e-15 * want, (text, float(m[0]), want)
+    # complex arguments: moduli
+    z = np.array([[0.3 - 0.4j]], dtype=CLD)
+    v, m = evaluate_with_magnitude(parse(block(1, [], "x[1]*x[1]-x[1]")), z, CLD)
+    assert abs(float(m[0]) - (0.25 + 0.5)) < 1e-15
+
+
+def test_magnitude_companion_is_sound_and_below_the_modulus_tree():
+    """FP64 evaluation of the same tree differs from the long-double value by far less than 1e-12 M
+    (soundness of the scale: the rounding unit is 1.1e-16), and M never exceeds R14's literal
+    modulus tree for expressions without quotients of cancelling arguments."""
+    rng = np.random.default_rng(12)
+    x = rng.uniform(0.01, 0.99, size=(4000, 3))
+    texts = ["(1-1.3*x[1]+x[2]*x[3])*(0.2-x[2]+x[1]*x[1])*l[1.01-x[3]]",
+             "p[1-1.9*x[1]*x[2]+x[3],-2.5]*(x[1]-x[2])/(1+x[3])",
+             "l[1+x[1]]*p[l[2-x[2]]-0.4,2]-p[x[3]-0.5,3]"]
+    for t in texts:
+        prog = parse(block(3, [], t))
+        v, m = evaluate_with_magnitude(prog, x)
+        d = evaluate(prog, x, np.float64)
+        ok = np.isfinite(v.astype(float))
+        assert ok.sum() > 3000
+        assert np.all(m[ok] >= np.abs(v[ok]) * (1 - 1e-18))
+        assert np.max(np.abs(d[ok] - v[ok].astype(float)) / m[ok].astype(float)) < 2e-14
+
+    def modulus_tree(node, xs):                                 # R14 literally, for + - * and positive powers
+        op = node[0]
+        if op == "num":
+            return np.full(xs.shape[0], abs(node[1]))
+        if op == "x":
+            return np.abs(xs[:, node[1] - 1])
+        if op == "neg":
+            return modulus_tree(node[1], xs)
+        if op in ("add", "sub"):
+            return modulus_tree(node[1], xs) + modulus_tree(node[2], xs)
+        if op == "mul":
+            return modulus_tree(node[1], xs) * modulus_tree(node[2], xs)
+        if op == "pow":
+            return modulus_tree(node[1], xs) ** int(node[2])
+        raise ValueError(op)
+
+    prog = parse(block(3, [], "(1-1.3*x[1]+x[2]*x[3])*p[0.2-x[2]+x[1]*x[1],3]-(x[1]-x[3])*(x[2]-0.5)"))
+    v, m = evaluate_with_magnitude(prog, x)
+    assert np.all(m.astype(float) <= modulus_tree(prog.final, x) * (1 + 1e-15))
+
+
+def test_fp64_horner_of_phi_r_errs_by_its_condition_number():
+    """DESIGN.md section 3 'Tolerances': the mirrored phi_r(v) = v^(r+1) sum_i c_i v^i, c_i =
+    C binom(r,i) (-1)^i/(r+1+i), is an alternating sum; its FP64 Horner value differs from the exact
+    one by about cond(v) = sum|c_i v^i| / |sum c_i v^i| rounding units, which is what sets the
+    4e-15 (r <= 4) / 4e-14 (r = 5, 6) bars of the GPU transform test.  FP64 Horner restated here."""
+    u64 = 2.0 ** -53
+    v = np.concatenate([np.linspace(1e-6, 0.5, 20001), 0.5 - np.logspace(-12, -2, 2000)])
+    for r in (3, 4, 5, 6):
+        C = math.factorial(2 * r + 1) // math.factorial(r) ** 2
+        coef = [C * math.comb(r, i) * (-1) ** i / (r + 1 + i) for i in range(r + 1)]
+        poly = np.full_like(v, coef[r])
+        for i in range(r - 1, -1, -1):
+            poly = poly * v + coef[i]                                  # numpy float64: one rounding per operation
+        exact = P._phi_small(v.astype(LD), r) / v.astype(LD) ** (r + 1)
+        rel = np.abs(poly - exact.astype(float)) / np.abs(exact.astype(float))
+        cond = sum(abs(c) * v ** i for i, c in enumerate(coef)) / np.abs(exact.astype(float))
+        assert np.all(rel <= 2 * (r + 2) * u64 * cond)                 # the standard Horner bound
+        assert cond.max() < {3: 13, 4: 33, 5: 90, 6: 250}[r]           # the condition numbers DESIGN.md quotes
+        # the polynomial alone, before the v^(r+1) factor and 1 - p add their roundings: inside the bars
+        assert rel.max() < (2.0e-15 if r <= 4 else 2.0e-14)
+        # r = 5, 6 do need the wider bar: the polynomial's own error is already above 4e-15
+        assert (rel.max() > 4e-15) == (r >= 5)
