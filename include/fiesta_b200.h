@@ -86,19 +86,29 @@ typedef struct {
 
 /* Parse, optimise, register-allocate and upload.  `info` may be NULL, else [nsectors].
  *
- * Two forms of the same instruction program are produced ("transforms to an internal
- * form"): (1) the fx_ins sequence, uploaded to the device arena and walked by the interpreter
- * kernels (all rules, real and complex); (2) for real sectors, that same sequence lowered
- * instruction by instruction to PTX, spliced into the evaluation kernel and assembled for sm_100a
- * in process -- one native kernel per sector, used by fiesta_integrate / fiesta_partial_sums with
- * the lattice rule when every selected sector has one.  Both forms perform the same operations in
- * the same order with the same roundings: their sums are bit-identical.  The environment variable
- * FIESTA_JIT=0 (read at each fiesta_compile) turns form (2) off. */
+ * Two forms of the same instruction program exist ("transforms to an internal form"):
+ *   (1) the fx_ins sequence, uploaded to the device arena and walked by the interpreter kernels.
+ *       It is complete when fiesta_compile returns: the program can be integrated at once.
+ *   (2) that same sequence lowered instruction by instruction to PTX, spliced into the evaluation
+ *       kernel and assembled for sm_100a in process: one native kernel per (sector, mode), mode =
+ *       a FIESTA_RULE_* or FIESTA_MODE_EVAL (real and complex sectors).  The program's own
+ *       background threads assemble them (~0.1-0.2 s of one host core per kernel): the lattice
+ *       rule's from fiesta_compile on, another mode's from the first call that uses it on.
+ * fiesta_integrate serves every sector with its native kernel if that is ready and with the
+ * interpreter otherwise; both forms perform the same operations in the same order with the same
+ * roundings, so a sector's sums are bit-identical whichever served it.
+ * Environment (read at each fiesta_compile): FIESTA_JIT=0 no native tier; FIESTA_JIT=sync return
+ * only when every sector's lattice kernel is ready; FIESTA_CACHE_DIR=<dir> keep assembled kernels
+ * on disk, keyed by the program (a process-wide in-memory cache always exists). */
 int fiesta_compile(fiesta_ctx *ctx, const fiesta_sector_desc *sectors, int32_t nsectors, int32_t dim,
                    fiesta_program **out, fiesta_compile_info *info);
 void fiesta_program_free(fiesta_program *prog);
 
 enum { FIESTA_RULE_LATTICE = 0, FIESTA_RULE_MC = 1, FIESTA_RULE_VEGAS = 2 };
+/* modes of the native kernels: the three rules, and the parity hook fiesta_eval_points */
+enum { FIESTA_MODE_EVAL = 3, FIESTA_N_MODES = 4 };
+/* tier arguments: whichever form is ready / interpreter only / native only (waits for the assembly) */
+enum { FIESTA_TIER_ANY = -1, FIESTA_TIER_INTERPRETER = 0, FIESTA_TIER_NATIVE = 1 };
 
 /* Sampling rule (R1-R4, R8; the paper names only "Vegas").
  *   LATTICE: npoints = n_shifts * N_L, N_L = 2^m; rank-1 lattice with generating vector genvec
@@ -136,17 +146,31 @@ int fiesta_integrate_async(fiesta_ctx *ctx, const fiesta_program *prog, const in
                            int32_t dim, uint64_t npoints, const fiesta_rule *rule, uint64_t seed);
 int fiesta_fetch_results(fiesta_ctx *ctx, int32_t nsectors, int32_t K, fiesta_result *out_host);
 
-/* Device time (ms, CUDA events on the ctx stream) that the evaluation kernel(s) of the last
- * fiesta_integrate[_async] took, and how many kernels the call launched.  Synchronises. */
+/* fiesta_integrate with the tier fixed (FIESTA_TIER_*).  out_host may be NULL (as _async). */
+int fiesta_integrate_tier(fiesta_ctx *ctx, const fiesta_program *prog, const int32_t *sectors, int32_t nsectors,
+                          int32_t dim, uint64_t npoints, const fiesta_rule *rule, uint64_t seed, int32_t tier,
+                          fiesta_result *out_host);
+
+/* Device time (ms, CUDA events on the ctx stream) that the evaluation kernels of the last
+ * fiesta_integrate[_async] took (chunk reductions between batches included), and how many kernels
+ * the call launched.  Synchronises. */
 int fiesta_last_timing(fiesta_ctx *ctx, double *eval_kernel_ms, int32_t *n_launches);
+
+/* How many (sector, pass) units of the last integrate-family call ran on a native kernel and how
+ * many on the interpreter. */
+int fiesta_last_tiers(fiesta_ctx *ctx, int32_t *n_native, int32_t *n_interpreter);
 
 /* ---- parity hooks: the same device code paths, exposed piecewise -------------------------- */
 
 /* Integrand values at caller-given points (PAPER.md:414 `justEvaluate`; PAPER.md:531 `Debug`).
  * x_host[npts][dim]; out_host[npts][K][2] = (re, im) of o_k(x) -- for deformed sectors
- * o_k(z(x)) * det J(x) -- WITHOUT the rule's weight. */
+ * o_k(z(x)) * det J(x) -- WITHOUT the rule's weight.  The native tier runs the sector's generated
+ * program body -- the text the integration kernels are assembled from -- in an eval kernel;
+ * fiesta_eval_points takes it when ready, _tier fixes the tier (FIESTA_TIER_NATIVE waits). */
 int fiesta_eval_points(fiesta_ctx *ctx, const fiesta_program *prog, int32_t sector, const double *x_host,
                        uint64_t npts, double *out_host);
+int fiesta_eval_points_tier(fiesta_ctx *ctx, const fiesta_program *prog, int32_t sector, int32_t tier,
+                            const double *x_host, uint64_t npts, double *out_host);
 
 /* The 64-bit integers t[j][k] (R2/R3) behind points j = first..first+count-1 of shift
  * (lattice) or iteration (MC/Vegas) `shift_or_iter` of the sector labelled sector_id.
@@ -166,12 +190,27 @@ int fiesta_transform_points(fiesta_ctx *ctx, const fiesta_rule *rule, const uint
 int fiesta_partial_sums(fiesta_ctx *ctx, const fiesta_program *prog, const int32_t *sectors, int32_t nsectors,
                         int32_t dim, uint64_t npoints, const fiesta_rule *rule, uint64_t seed,
                         double *sums_host);
+int fiesta_partial_sums_tier(fiesta_ctx *ctx, const fiesta_program *prog, const int32_t *sectors, int32_t nsectors,
+                             int32_t dim, uint64_t npoints, const fiesta_rule *rule, uint64_t seed, int32_t tier,
+                             double *sums_host);
+
+/* The first level of the two-level reduction: the partial record of every block.  A block sums the
+ * points j = c * chunk_points .. min((c+1) * chunk_points, N_L) - 1 of one (sector, shift), c <
+ * nchunks.  sums_host[nsectors][R][nchunks][K][C][2]; with sums_host == NULL only the geometry is
+ * returned.  For sampled checks of a full-size launch: the chunking is that of fiesta_integrate for
+ * the same rule and npoints.  nsectors must fit one batch (FIESTA_E_ARG otherwise). */
+int fiesta_chunk_sums(fiesta_ctx *ctx, const fiesta_program *prog, const int32_t *sectors, int32_t nsectors,
+                      int32_t dim, uint64_t npoints, const fiesta_rule *rule, uint64_t seed, int32_t tier,
+                      uint64_t *chunk_points, int32_t *nchunks, double *sums_host);
 
 /* One Vegas iteration of one sector on a caller-given grid (R8):
  * grid_host[dim][NB+1] in; sums_host[K][C][2] (S1, S2) and hist_host[dim][NB] out. */
 int fiesta_vegas_iteration(fiesta_ctx *ctx, const fiesta_program *prog, int32_t sector, int32_t dim,
                            uint64_t npoints, const fiesta_rule *rule, uint64_t seed, int32_t iteration,
                            const double *grid_host, double *sums_host, double *hist_host);
+int fiesta_vegas_iteration_tier(fiesta_ctx *ctx, const fiesta_program *prog, int32_t sector, int32_t dim,
+                                uint64_t npoints, const fiesta_rule *rule, uint64_t seed, int32_t iteration,
+                                int32_t tier, const double *grid_host, double *sums_host, double *hist_host);
 
 /* The grid refinement step alone: ngrids independent (grid[NB+1], hist[NB]) pairs. */
 int fiesta_vegas_refine(fiesta_ctx *ctx, int32_t ngrids, int32_t nbins, double alpha, const double *grid_host,
@@ -186,17 +225,29 @@ int fiesta_vegas_grid(fiesta_ctx *ctx, int32_t sector, int32_t dim, int32_t nbin
  * nsectors*K numbers; total_host[K]. */
 int fiesta_combine(const fiesta_result *per_sector_host, int32_t nsectors, int32_t K, fiesta_result *total_host);
 
-/* 1 if `sector` has a native kernel (form 2 above), else 0 with the reason in why_host (may be
- * NULL; "" when the native tier is switched off or does not apply); <0 on bad arguments. */
-int fiesta_program_native(const fiesta_program *prog, int32_t sector, char *why_host, uint64_t buflen);
+/* 1 if the native kernel of (`sector`, `mode`) is ready, else 0; <0 on bad arguments.  info_host (may
+ * be NULL) receives, when ready, the assembler's resource report ("Used N registers, ... bytes spill
+ * stores ..."), else why not ("" = never requested or the native tier is off, "being assembled",
+ * or the assembler's error). */
+int fiesta_program_native(const fiesta_program *prog, int32_t sector, int32_t mode, char *info_host, uint64_t buflen);
 
-/* Host only (no context, no GPU): compile one real sector and run the native tier's lowering and
- * assembly on it.  Writes the generated PTX (the .const array of the program's FP64 immediates, then
- * the program body; NUL-terminated, truncated to buflen) to ptx_body_host (may be NULL) and the
- * size of the assembled sm_100a cubin to cubin_bytes (may be NULL).  FIESTA_E_ARG for complex sectors; FIESTA_E_PARSE etc. as
- * fiesta_compile; FIESTA_E_CUDA if the PTX assembler rejects the module (message in ptx_body_host). */
-int fiesta_native_assemble(const fiesta_sector_desc *sector, int32_t dim, char *ptx_body_host, uint64_t buflen,
-                           uint64_t *cubin_bytes);
+/* Request the `mode` kernels of all sectors and wait (timeout_s < 0: for ever) until none is queued or
+ * being assembled.  Returns how many are ready, or <0. */
+int fiesta_program_wait_native(fiesta_program *prog, int32_t mode, double timeout_s);
+
+/* Background assembly so far: kernels assembled, kernels taken from the cache, host-core seconds
+ * spent (summed over the program's threads), number of threads.  Any pointer may be NULL. */
+int fiesta_program_native_stats(const fiesta_program *prog, int32_t *n_assembled, int32_t *n_cache_hits,
+                                double *assemble_cpu_seconds, int32_t *n_threads);
+
+/* Host only (no context, no GPU): compile one sector and run the native tier's lowering and assembly
+ * on it for `mode`.  Writes the generated PTX (the .const array of the program's FP64 immediates, then
+ * the program body or bodies; NUL-terminated, truncated to buflen) to ptx_body_host (may be NULL), the
+ * size of the assembled sm_100a cubin to cubin_bytes (may be NULL) and the assembler's resource report
+ * to info_host (may be NULL).  FIESTA_E_PARSE etc. as fiesta_compile; FIESTA_E_CUDA if the PTX
+ * assembler rejects the module (message in ptx_body_host). */
+int fiesta_native_assemble(const fiesta_sector_desc *sector, int32_t dim, int32_t mode, char *ptx_body_host,
+                           uint64_t buflen, uint64_t *cubin_bytes, char *info_host, uint64_t infolen);
 
 /* Disassembly of a compiled sector (main program, then the deformation program) into buf. */
 int fiesta_program_dump(const fiesta_program *prog, int32_t sector, char *buf_host, uint64_t buflen);

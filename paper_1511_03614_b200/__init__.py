@@ -7,7 +7,8 @@ raise.
 """
 from .binding import (  # noqa: F401
     Context, Program, Rule, FiestaError, LIB_PATH, load_library, exported_symbols, native_assemble,
-    RULE_LATTICE, RULE_MC, RULE_VEGAS, RESULT_DTYPE, INFO_DTYPE,
+    RULE_LATTICE, RULE_MC, RULE_VEGAS, MODE_EVAL, N_MODES, TIER_ANY, TIER_INTERPRETER, TIER_NATIVE,
+    RESULT_DTYPE, INFO_DTYPE,
 )
 
 load = load_library

@@ -10,6 +10,8 @@ import numpy as np
 LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libfiesta_b200.so")
 
 RULE_LATTICE, RULE_MC, RULE_VEGAS = 0, 1, 2
+MODE_EVAL, N_MODES = 3, 4
+TIER_ANY, TIER_INTERPRETER, TIER_NATIVE = -1, 0, 1
 MAX_ORDERS = 8
 
 RESULT_DTYPE = np.dtype([("re", "f8"), ("re_err", "f8"), ("im", "f8"), ("im_err", "f8"), ("chi2", "f8"),
@@ -62,8 +64,18 @@ _SIGNATURES = {
     "fiesta_vegas_grid": (C.c_int, [_VP, _I32, _I32, _I32, _VP, _VP]),
     "fiesta_combine": (C.c_int, [_VP, _I32, _I32, _VP]),
     "fiesta_program_dump": (C.c_int, [_VP, _I32, C.c_char_p, _U64]),
-    "fiesta_program_native": (C.c_int, [_VP, _I32, C.c_char_p, _U64]),
-    "fiesta_native_assemble": (C.c_int, [_VP, _I32, C.c_char_p, _U64, C.POINTER(_U64)]),
+    "fiesta_program_native": (C.c_int, [_VP, _I32, _I32, C.c_char_p, _U64]),
+    "fiesta_program_wait_native": (C.c_int, [_VP, _I32, C.c_double]),
+    "fiesta_program_native_stats": (C.c_int, [_VP, C.POINTER(_I32), C.POINTER(_I32), C.POINTER(C.c_double), C.POINTER(_I32)]),
+    "fiesta_native_assemble": (C.c_int, [_VP, _I32, _I32, C.c_char_p, _U64, C.POINTER(_U64), C.c_char_p, _U64]),
+    "fiesta_integrate_tier": (C.c_int, [_VP, _VP, _VP, _I32, _I32, _U64, C.POINTER(_Rule), _U64, _I32, _VP]),
+    "fiesta_last_tiers": (C.c_int, [_VP, C.POINTER(_I32), C.POINTER(_I32)]),
+    "fiesta_eval_points_tier": (C.c_int, [_VP, _VP, _I32, _I32, _VP, _U64, _VP]),
+    "fiesta_partial_sums_tier": (C.c_int, [_VP, _VP, _VP, _I32, _I32, _U64, C.POINTER(_Rule), _U64, _I32, _VP]),
+    "fiesta_chunk_sums": (C.c_int, [_VP, _VP, _VP, _I32, _I32, _U64, C.POINTER(_Rule), _U64, _I32, C.POINTER(_U64),
+                                    C.POINTER(_I32), _VP]),
+    "fiesta_vegas_iteration_tier": (C.c_int, [_VP, _VP, _I32, _I32, _U64, C.POINTER(_Rule), _U64, _I32, _I32, _VP, _VP,
+                                              _VP]),
     "fiesta_fp64_peak": (C.c_int, [_VP, C.c_double, C.POINTER(C.c_double)]),
 }
 
@@ -122,19 +134,21 @@ def _ptr(a):
     return None if a is None else a.ctypes.data_as(_VP)
 
 
-def native_assemble(sector, dim, buflen=1 << 22):
+def native_assemble(sector, dim, mode=RULE_LATTICE, buflen=1 << 23):
     """fiesta_native_assemble: host only.  sector: object with .sector_id, .texts (workloads.SectorText).
-    -> (generated PTX of the program body, bytes of the assembled sm_100a cubin)."""
+    -> (generated PTX of the program body/bodies, bytes of the assembled sm_100a cubin, the assembler's
+    resource report)."""
     lib = load_library()
     arr = (C.c_char_p * len(sector.texts))(*[t.encode() for t in sector.texts])
     d = _SectorDesc(int(sector.sector_id), len(sector.texts), C.cast(arr, C.POINTER(C.c_char_p)),
                     int(bool(sector.is_complex)), int(sector.deform_f_index), float(sector.lam))
     buf = C.create_string_buffer(buflen)
+    info = C.create_string_buffer(1 << 14)
     n = _U64(0)
-    rc = lib.fiesta_native_assemble(C.byref(d), int(dim), buf, buflen, C.byref(n))
+    rc = lib.fiesta_native_assemble(C.byref(d), int(dim), int(mode), buf, buflen, C.byref(n), info, 1 << 14)
     if rc != 0:
         raise FiestaError(rc, buf.value.decode(errors="replace"))
-    return buf.value.decode(), int(n.value)
+    return buf.value.decode(), int(n.value), info.value.decode(errors="replace")
 
 
 class Program:
@@ -151,13 +165,27 @@ class Program:
 
     __del__ = close
 
-    def native(self, sector=0):
-        """(has a native kernel, reason if not) -- fiesta_program_native"""
-        buf = C.create_string_buffer(4096)
-        rc = load_library().fiesta_program_native(self.handle, sector, buf, 4096)
+    def native(self, sector=0, mode=RULE_LATTICE):
+        """(the native kernel of (sector, mode) is ready, the assembler's report or the reason if not)
+        -- fiesta_program_native"""
+        buf = C.create_string_buffer(1 << 14)
+        rc = load_library().fiesta_program_native(self.handle, sector, mode, buf, 1 << 14)
         if rc < 0:
             raise FiestaError(rc, "fiesta_program_native")
-        return bool(rc), buf.value.decode()
+        return bool(rc), buf.value.decode(errors="replace")
+
+    def wait_native(self, mode=RULE_LATTICE, timeout_s=-1.0):
+        """Request the `mode` kernels of all sectors and wait for the background assembly; -> number ready."""
+        rc = load_library().fiesta_program_wait_native(self.handle, int(mode), float(timeout_s))
+        if rc < 0:
+            raise FiestaError(rc, "fiesta_program_wait_native")
+        return rc
+
+    def native_stats(self):
+        """-> dict(assembled, cache_hits, cpu_seconds, threads) of the background assembly so far."""
+        a, h, t, n = _I32(), _I32(), C.c_double(), _I32()
+        load_library().fiesta_program_native_stats(self.handle, C.byref(a), C.byref(h), C.byref(t), C.byref(n))
+        return dict(assembled=a.value, cache_hits=h.value, cpu_seconds=t.value, threads=n.value)
 
     def dump(self, sector=0, buflen=1 << 20):
         buf = C.create_string_buffer(buflen)
@@ -216,15 +244,27 @@ class Context:
         a = np.ascontiguousarray(sectors, dtype=np.int32)
         return a, len(a), [int(i) for i in a]
 
-    def integrate(self, prog, npoints, rule, seed, sectors=None, allow_nonfinite=False):
-        """-> numpy record array [nsectors][K] of RESULT_DTYPE."""
+    def integrate(self, prog, npoints, rule, seed, sectors=None, allow_nonfinite=False, tier=None):
+        """-> numpy record array [nsectors][K] of RESULT_DTYPE.  tier: None (fiesta_integrate: whichever form
+        of each sector is ready) or TIER_INTERPRETER / TIER_NATIVE (fiesta_integrate_tier)."""
         sel, nsel, idx = self._sel(prog, sectors)
         K = prog.K[idx[0]]
         out = np.zeros((nsel, K), dtype=RESULT_DTYPE)
         r, keep = rule._c()
-        self._check(self.lib.fiesta_integrate(self.handle, prog.handle, _ptr(sel), nsel, prog.dim, int(npoints),
-                                              C.byref(r), int(seed), _ptr(out)), allow_nonfinite)
+        if tier is None:
+            rc = self.lib.fiesta_integrate(self.handle, prog.handle, _ptr(sel), nsel, prog.dim, int(npoints),
+                                           C.byref(r), int(seed), _ptr(out))
+        else:
+            rc = self.lib.fiesta_integrate_tier(self.handle, prog.handle, _ptr(sel), nsel, prog.dim, int(npoints),
+                                                C.byref(r), int(seed), int(tier), _ptr(out))
+        self._check(rc, allow_nonfinite)
         return out
+
+    def last_tiers(self):
+        """(sector passes of the last call served by a native kernel, by the interpreter)"""
+        a, b = _I32(), _I32()
+        self._check(self.lib.fiesta_last_tiers(self.handle, C.byref(a), C.byref(b)))
+        return a.value, b.value
 
     def integrate_async(self, prog, npoints, rule, seed, sectors=None):
         sel, nsel, _ = self._sel(prog, sectors)
@@ -243,12 +283,17 @@ class Context:
         return ms.value, n.value
 
     # ---- parity hooks --------------------------------------------------------------------
-    def eval_points(self, prog, sector, x):
+    def eval_points(self, prog, sector, x, tier=None):
         """x [npts][dim] float64 -> complex128 [npts][K] (weight excluded)."""
         x = np.ascontiguousarray(x, dtype=np.float64).reshape(-1, prog.dim)
         K = prog.K[sector]
         out = np.zeros((x.shape[0], K, 2), dtype=np.float64)
-        self._check(self.lib.fiesta_eval_points(self.handle, prog.handle, int(sector), _ptr(x), x.shape[0], _ptr(out)))
+        if tier is None:
+            rc = self.lib.fiesta_eval_points(self.handle, prog.handle, int(sector), _ptr(x), x.shape[0], _ptr(out))
+        else:
+            rc = self.lib.fiesta_eval_points_tier(self.handle, prog.handle, int(sector), int(tier), _ptr(x), x.shape[0],
+                                                  _ptr(out))
+        self._check(rc)
         return out[..., 0] + 1j * out[..., 1]
 
     def generate_points(self, rule, seed, sector_id, shift_or_iter, n_lattice, first, count, dim):
@@ -268,26 +313,40 @@ class Context:
                                                      _ptr(xbar), _ptr(w)))
         return x, xbar, w
 
-    def partial_sums(self, prog, npoints, rule, seed, sectors=None):
+    def partial_sums(self, prog, npoints, rule, seed, sectors=None, tier=TIER_ANY):
         """-> float64 [nsectors][R][K][C][2] (S1, S2); all selected sectors must share K and C."""
         sel, nsel, idx = self._sel(prog, sectors)
         K, cc = prog.K[idx[0]], 2 if prog.is_complex[idx[0]] else 1
         R = rule.n_shifts if rule.kind == RULE_LATTICE else 1
         out = np.zeros((nsel, R, K, cc, 2), dtype=np.float64)
         r, keep = rule._c()
-        self._check(self.lib.fiesta_partial_sums(self.handle, prog.handle, _ptr(sel), nsel, prog.dim, int(npoints),
-                                                 C.byref(r), int(seed), _ptr(out)))
+        self._check(self.lib.fiesta_partial_sums_tier(self.handle, prog.handle, _ptr(sel), nsel, prog.dim, int(npoints),
+                                                      C.byref(r), int(seed), int(tier), _ptr(out)))
         return out
 
-    def vegas_iteration(self, prog, sector, npoints, rule, seed, iteration, grid):
+    def chunk_sums(self, prog, npoints, rule, seed, sectors=None, tier=TIER_ANY):
+        """-> (chunk_points, float64 [nsectors][R][nchunks][K][C][2]): every block's partial record."""
+        sel, nsel, idx = self._sel(prog, sectors)
+        K, cc = prog.K[idx[0]], 2 if prog.is_complex[idx[0]] else 1
+        R = rule.n_shifts if rule.kind == RULE_LATTICE else 1
+        r, keep = rule._c()
+        cp, nch = _U64(), _I32()
+        args = (self.handle, prog.handle, _ptr(sel), nsel, prog.dim, int(npoints), C.byref(r), int(seed), int(tier),
+                C.byref(cp), C.byref(nch))
+        self._check(self.lib.fiesta_chunk_sums(*args, None))
+        out = np.zeros((nsel, R, nch.value, K, cc, 2), dtype=np.float64)
+        self._check(self.lib.fiesta_chunk_sums(*args, _ptr(out)))
+        return int(cp.value), out
+
+    def vegas_iteration(self, prog, sector, npoints, rule, seed, iteration, grid, tier=TIER_ANY):
         grid = np.ascontiguousarray(grid, dtype=np.float64)
         K, cc = prog.K[sector], 2 if prog.is_complex[sector] else 1
         sums = np.zeros((K, cc, 2))
         hist = np.zeros((prog.dim, rule.vegas_bins))
         r, keep = rule._c()
-        self._check(self.lib.fiesta_vegas_iteration(self.handle, prog.handle, int(sector), prog.dim, int(npoints),
-                                                    C.byref(r), int(seed), int(iteration), _ptr(grid), _ptr(sums),
-                                                    _ptr(hist)))
+        self._check(self.lib.fiesta_vegas_iteration_tier(self.handle, prog.handle, int(sector), prog.dim, int(npoints),
+                                                         C.byref(r), int(seed), int(iteration), int(tier), _ptr(grid),
+                                                         _ptr(sums), _ptr(hist)))
         return sums, hist
 
     def vegas_refine(self, grid, hist, alpha):

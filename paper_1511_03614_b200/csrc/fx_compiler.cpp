@@ -1056,6 +1056,7 @@ CompiledSector compile_sector(const char *const *texts, int K, int dim, bool is_
   cs.is_complex = is_complex || deform_f_index > 0;
   cs.deform_on = deform_f_index > 0;
   cs.lambda = lambda;
+  if (deform_f_index > 0 && !(lambda >= 0.0)) fail(FIESTA_E_ARG, "lambda must be >= 0 (PAPER.md:474: Im F(z) < 0 needs a positive deformation)");
 
   Lowering low(raw, fbound, dim);
   std::vector<int> lroots(K);

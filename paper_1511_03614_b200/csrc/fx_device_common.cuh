@@ -25,11 +25,11 @@ __host__ __device__ inline fx_smem_layout fx_layout(int prog_ins, int mem_double
   L.delta = o;
   o += FX_NXMAX * 8u;
   L.tf = o;
-  o += 80u;  // fx_transform (80 bytes), kept in shared memory for the per-coordinate helper
+  o += FX_TF_BYTES;  // fx_transform (80 bytes) for the per-coordinate helper, then the lattice steps G_k
   L.grid = o;
   o += vegas ? (uint32_t)dim * (nbins + 1) * 8u : 0u;
   L.hist = o;
-  o += vegas ? (uint32_t)dim * nbins * 8u : 0u;
+  o += vegas ? (FX_THREADS / 32) * (uint32_t)dim * nbins * 8u : 0u;  // one histogram per warp
   L.wsum = o;
   o += FX_ACC_SLOTS * (FX_THREADS / 32) * 8u;
   L.total = o;
@@ -40,6 +40,15 @@ __device__ __forceinline__ void fx_copy_program(fx_ins *dst, const fx_ins *src, 
   const uint4 *s = reinterpret_cast<const uint4 *>(src);
   uint4 *d = reinterpret_cast<uint4 *>(dst);
   for (int i = threadIdx.x; i < n; i += blockDim.x) d[i] = s[i];
+}
+
+// the lattice steps G_k live in shared memory behind the transform (fx_layout / fxj_layout): loop
+// invariants the evaluation kernels need not hold in registers across the program walk
+__device__ __forceinline__ uint64_t *fx_lattice_steps(uint64_t *sh_delta) {
+  return sh_delta + FX_NXMAX + 80 / 8;
+}
+__device__ __forceinline__ const uint64_t *fx_lattice_steps(const uint64_t *sh_delta) {
+  return sh_delta + FX_NXMAX + 80 / 8;
 }
 
 // Out-of-line helpers: the evaluation kernels call them once per coordinate.  Keeping one copy of
@@ -112,7 +121,7 @@ __device__ __forceinline__ void fx_make_points(const fx_integrate_params &prm, i
     for (int k = 0; k < NX; ++k) {
       if (k < dim) {
         // t_j = ((j g) mod 2^m) << (64-m) + Delta = j * (g << (64-m)) + Delta  (mod 2^64)
-        const uint64_t G = prm.log2_n ? (prm.genvec[k] << (64 - prm.log2_n)) : 0ull;
+        const uint64_t G = fx_lattice_steps(sh_delta)[k];
         fx_tP<P> tt;
         FX_PLOOP { tt.t[p] = (j0 + p) * G + sh_delta[k]; }
         const fx_coordP<P> c = fx_lattice_coord<P>(tt, tf);
@@ -173,6 +182,9 @@ __device__ __forceinline__ void fx_block_setup(const fx_integrate_params &prm, i
     sh_delta[2 * threadIdx.x] = te;
     sh_delta[2 * threadIdx.x + 1] = to;
   }
+  if (threadIdx.x >= 64 && threadIdx.x < 64 + FX_NXMAX)  // t_j = j * G_k + Delta_k (mod 2^64), G_k = g_k << (64-m)
+    fx_lattice_steps(sh_delta)[threadIdx.x - 64] =
+        (prm.rule == FIESTA_RULE_LATTICE && prm.log2_n) ? (prm.genvec[threadIdx.x - 64] << (64 - prm.log2_n)) : 0ull;
   if (threadIdx.x == 32) {  // fx_layout puts the transform right after the shifts
     fx_transform *tf = reinterpret_cast<fx_transform *>(sh_delta + FX_NXMAX);
     tf->r = prm.tf.r;
@@ -185,7 +197,43 @@ __device__ __forceinline__ void fx_block_setup(const fx_integrate_params &prm, i
   if (prm.rule == FIESTA_RULE_VEGAS) {
     const double *g = prm.grid + (size_t)sel_idx * dim * (prm.nbins + 1);
     for (int i = threadIdx.x; i < dim * (prm.nbins + 1); i += blockDim.x) sh_grid[i] = g[i];
-    for (int i = threadIdx.x; i < dim * prm.nbins; i += blockDim.x) sh_hist[i] = 0.0;
+    for (int i = threadIdx.x; i < (FX_THREADS / 32) * dim * prm.nbins; i += blockDim.x) sh_hist[i] = 0.0;
+  }
+}
+
+// Vegas histogram (R8): h[k][bin] += v for one point per lane, into the
+// WARP's own histogram in shared memory.  Warp-aggregated: lanes whose points fall into the same bin
+// are found with match.any and their values are added in lane order by every lane of the group; the
+// group's first lane then does one plain read-modify-write.  No atomics, and the order of every
+// addition is fixed, so the histogram -- like the sums -- is bit-reproducible.
+__device__ __forceinline__ void fx_hist_add(double *warp_hist_k /* this warp's h[k][0..nbins) */, unsigned bin,
+                                            double v, bool valid) {
+  const unsigned full = 0xffffffffu;
+  const unsigned lane = threadIdx.x & 31u;
+  const unsigned key = valid ? bin : (0x100u | lane);  // a point past the end matches nobody
+  const unsigned peers = __match_any_sync(full, key);
+  const unsigned maxn = __reduce_max_sync(full, (unsigned)__popc(peers));
+  double sum = 0.0;
+  unsigned m = peers;
+  for (unsigned it = 0; it < maxn; ++it) {
+    const int src = m ? (__ffs(m) - 1) : (int)lane;
+    const double t = __shfl_sync(full, v, src);
+    if (m) sum += t;
+    m &= m - 1;
+  }
+  if (valid && lane == (unsigned)(__ffs(peers) - 1)) warp_hist_k[bin] += sum;
+  __syncwarp();
+}
+
+// all dimensions of the P points of a thread, point by point (the order both tiers use)
+template <int NX, int P>
+__device__ __forceinline__ void fx_hist_points(double *sh_hist, int dim, int nbins, unsigned valid,
+                                               const uint32_t (&bins)[(NX + 3) / 4][P], const double (&h2)[P]) {
+  double *wh = sh_hist + (size_t)(threadIdx.x >> 5) * dim * nbins;
+  FX_PLOOP {
+#pragma unroll
+    for (int k = 0; k < NX; ++k)
+      if (k < dim) fx_hist_add(wh + k * nbins, (bins[k / 4][p] >> (8 * (k % 4))) & 0xffu, h2[p], (valid >> p) & 1u);
   }
 }
 
@@ -199,25 +247,53 @@ __device__ __forceinline__ void fx_block_reduce(const double *sh_acc, double *sh
     if (lane == 0) sh_wsum[s * (FX_THREADS / 32) + warp] = v;
   }
   __syncthreads();
-  if (threadIdx.x < nslots) {
+  if (threadIdx.x < FX_ACC_SLOTS) {  // every slot of the record is written: the buffer is never cleared
     double t = 0.0;
-    for (int w = 0; w < FX_THREADS / 32; ++w) t += sh_wsum[threadIdx.x * (FX_THREADS / 32) + w];
+    if (threadIdx.x < nslots)
+      for (int w = 0; w < FX_THREADS / 32; ++w) t += sh_wsum[threadIdx.x * (FX_THREADS / 32) + w];
     out[threadIdx.x] = t;
   }
 }
 
-__device__ __forceinline__ void fx_block_finish(const fx_integrate_params &prm, int dim, int sel_idx, unsigned nonfinite,
-                                                const double *sh_hist) {
+// block end: non-finite count (an integer: atomics keep it exact), and the block's histogram = the
+// warps' histograms added in warp order, written to this block's own record (fx_launch_reduce_hist
+// adds the records in block order)
+__device__ __forceinline__ void fx_block_finish(const fx_integrate_params &prm, int dim, int sel_idx, int chunk,
+                                                unsigned nonfinite, const double *sh_hist) {
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) nonfinite += __shfl_down_sync(0xffffffffu, nonfinite, off);
   if ((threadIdx.x & 31) == 0 && nonfinite) atomicAdd(prm.nonfinite + sel_idx, (unsigned long long)nonfinite);
   if (prm.rule == FIESTA_RULE_VEGAS) {
-    double *h = prm.hist + (size_t)sel_idx * dim * prm.nbins;
-    for (int i = threadIdx.x; i < dim * prm.nbins; i += blockDim.x) {
-      double v = sh_hist[i];
-      if (v != 0.0) atomicAdd(h + i, v);
+    const int cells = dim * prm.nbins;
+    double *h = prm.hist_part + ((size_t)(sel_idx - prm.batch_base) * prm.nchunks + chunk) * cells;
+    __syncthreads();
+    for (int i = threadIdx.x; i < cells; i += blockDim.x) {
+      double v = 0.0;
+      for (int w = 0; w < FX_THREADS / 32; ++w) v += sh_hist[w * cells + i];
+      h[i] = v;
     }
   }
+}
+
+// Which (sector, shift, chunk) this block works on.  The block index is read through a volatile asm,
+// so a kernel that asks again after its point loop gets a recomputation there instead of three
+// registers held (or spilled to local memory) across the whole program walk.
+struct fx_block_id {
+  int chunk, r, sel_idx;
+};
+__device__ __forceinline__ fx_block_id fx_block_coords(const fx_integrate_params &prm) {
+  unsigned b;
+  asm volatile("mov.u32 %0, %%ctaid.x;" : "=r"(b));
+  fx_block_id id;
+  id.chunk = (int)(b % (unsigned)prm.nchunks);
+  id.r = (int)((b / (unsigned)prm.nchunks) % (unsigned)prm.n_shifts);
+  id.sel_idx = fx_sel_index(prm, (int)(b / ((unsigned)prm.nchunks * (unsigned)prm.n_shifts)));
+  return id;
+}
+
+// where this block's partial record goes
+__device__ __forceinline__ double *fx_partial_record(const fx_integrate_params &prm, int sel_idx, int r, int chunk) {
+  return prm.partials + (((size_t)(sel_idx - prm.batch_base) * prm.n_shifts + r) * prm.nchunks + chunk) * FX_ACC_SLOTS;
 }
 
 #endif

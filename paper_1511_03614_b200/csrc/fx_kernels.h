@@ -10,6 +10,7 @@
 #define FX_THREADS 128   // threads per block of the evaluation kernels
 #define FX_P_REAL 4      // points per thread, real programs
 #define FX_P_CPLX 1      // points per thread, complex programs
+#define FX_TF_BYTES (80u + FX_NXMAX * 8u)  // shared memory: fx_transform, then the lattice steps G_k
 #define FX_ACC_SLOTS 32  // per-(sector,shift,chunk) partial record: [K<=8][C<=2][S1,S2]
 
 struct fx_sector_dev {       // one compiled sector in the device arena
@@ -50,13 +51,26 @@ struct fx_integrate_params {
   uint64_t seed;
   int32_t nbins;
   const double *grid;        // Vegas: [nsel][dim][nbins+1]
-  double *hist;              // Vegas: [nsel][dim][nbins]
-  double *partials;          // [nsel][R][nchunks][FX_ACC_SLOTS]
+  double *hist_part;         // Vegas: per-block histograms of this batch [batch sector][nchunks][dim][nbins]
+  double *partials;          // partial records of this batch [batch sector][R][nchunks][FX_ACC_SLOTS]
   unsigned long long *nonfinite;  // [nsel]
   int32_t mem_doubles;       // shared-memory spill doubles per block (all threads)
   int32_t prog_ins_max;      // instructions reserved in shared memory (main + deform)
-  int32_t sel_base;          // native per-sector kernels (fx_jit): index into sel of the launch's first sector
+  // A launch covers some sectors of one batch of the call (a batch = consecutive positions
+  // batch_base .. of the selection; its partial records are what `partials` / `hist_part` point to).
+  // Block q / (nchunks * n_shifts) = launch-local sector number j; its position in the selection is
+  // launch_map[j] (interpreter launches over the sectors of the batch that have no native kernel yet)
+  // or sel_base + j when launch_map is NULL (one native kernel per sector).
+  const int32_t *launch_map;
+  int32_t sel_base;
+  int32_t batch_base;        // position in the selection of the batch's first sector
+  unsigned long long *testf; // [nsel]: points with Im F(z) >= 0 (deformed sectors; PAPER.md:474 -testF), or NULL
 };
+
+// position in the selection of the sector a block works on
+static inline __host__ __device__ int fx_sel_index(const fx_integrate_params &prm, int launch_sector) {
+  return prm.launch_map ? prm.launch_map[launch_sector] : prm.sel_base + launch_sector;
+}
 
 struct fx_eval_params {
   const fx_ins *arena;
@@ -71,28 +85,33 @@ struct fx_eval_params {
 };
 
 size_t fx_integrate_smem_bytes(const fx_integrate_params &p);
-size_t fx_integrate_smem_bytes_native(int dim);  // native per-sector kernels: no program, no spill slots
 
-// Shared-memory layout of the native kernels (fx_jit_template.cu): accumulators for K <= 8 real
-// outputs (sum g, sum g^2: 16 slots, one column per thread), the lattice shifts, the transform
-// parameters (fx_block_setup puts them right after the shifts), the block reduction's per-warp sums.
-#define FXJ_ACC_SLOTS 16
+// Shared-memory layout of the native kernels (fx_jit_template*.cu): accumulators (sum g, sum g^2 per
+// output component: FXJ_ACC_SLOTS slots, one column per thread), the lattice shifts, the transform
+// parameters (fx_block_setup puts them right after the shifts), Vegas grid and per-warp histograms,
+// the block reduction's per-warp sums.  No program and no spill slots: both are registers.
+#define FXJ_ACC_SLOTS 32
 #define FXJ_P 2  // points per thread and pass of the native program body (two passes per batch of FX_P_REAL)
 struct fxj_smem_layout {
-  uint32_t acc, delta, tf, wsum, total;
+  uint32_t acc, delta, tf, grid, hist, wsum, total;
 };
-static inline __host__ __device__ fxj_smem_layout fxj_layout() {
+static inline __host__ __device__ fxj_smem_layout fxj_layout(int dim, int nbins, bool vegas, int acc_slots = 16) {
   fxj_smem_layout L;
   L.acc = 0;
-  L.delta = FXJ_ACC_SLOTS * FX_THREADS * 8u;
+  L.delta = (uint32_t)acc_slots * FX_THREADS * 8u;
   L.tf = L.delta + FX_NXMAX * 8u;
-  L.wsum = L.tf + 80u;
-  L.total = L.wsum + FXJ_ACC_SLOTS * (FX_THREADS / 32) * 8u;
+  L.grid = L.tf + FX_TF_BYTES;
+  L.hist = L.grid + (vegas ? (uint32_t)dim * (nbins + 1) * 8u : 0u);
+  L.wsum = L.hist + (vegas ? (FX_THREADS / 32) * (uint32_t)dim * nbins * 8u : 0u);
+  L.total = L.wsum + (uint32_t)acc_slots * (FX_THREADS / 32) * 8u;
   return L;
 }
 
-// S[nsel][R][FX_ACC_SLOTS] = sum over chunks of the partials, fixed order
-cudaError_t fx_launch_reduce_chunks(const double *partials, double *sums, int nsel, int R, int nchunks, cudaStream_t st);
+// S[row][FX_ACC_SLOTS] = sum over chunks of the partials of nrows (sector, shift) rows, fixed order
+cudaError_t fx_launch_reduce_chunks(const double *partials, double *sums, int nrows, int nchunks, cudaStream_t st);
+// Vegas: hist[sector][dim*nbins] = sum over the blocks' histograms, fixed order
+cudaError_t fx_launch_reduce_hist(const double *hist_part, double *hist, int nsectors, int nchunks, int cells,
+                                  cudaStream_t st);
 
 struct fx_result_dev {
   double re, re_err, im, im_err, chi2;

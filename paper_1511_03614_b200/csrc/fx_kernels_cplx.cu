@@ -11,6 +11,7 @@
 #endif
 #define FX_WANT(is_cplx, nx, p) ((nx) == FX_N && (p) == 1)  // real (deformation program) and complex, P = 2
 #include "fx_device_common.cuh"
+#include "fx_deform.cuh"
 
 #define FX_CAT2(a, b) a##b
 #define FX_CAT(a, b) FX_CAT2(a, b)
@@ -25,45 +26,6 @@ constexpr int NGH = N + N * (N + 1) / 2;  // gradient + upper Hessian slots writ
 struct NoSink {
   __device__ __forceinline__ void operator()(int, double (&)[P]) {}
 };
-
-__device__ __forceinline__ int hess_slot(int k, int l) {  // k <= l, row-major upper triangle after the gradient
-  return N + k * N - k * (k - 1) / 2 + (l - k);
-}
-
-// det of J (complex N x N, registers) by LU with partial pivoting on |.|^2 (R12)
-__device__ __forceinline__ cplx det_lu(cplx (&J)[N][N]) {
-  cplx det{1.0, 0.0};
-#pragma unroll
-  for (int c = 0; c < N; ++c) {
-#pragma unroll
-    for (int r = c + 1; r < N; ++r) {
-      const double mc = fma(J[c][c].re, J[c][c].re, J[c][c].im * J[c][c].im);
-      const double mr = fma(J[r][c].re, J[r][c].re, J[r][c].im * J[r][c].im);
-      // row exchange by value selects (a branch around array element swaps keeps J in local memory)
-      const bool sw = mr > mc;
-#pragma unroll
-      for (int l = c; l < N; ++l) {
-        const cplx a = J[c][l], b = J[r][l];
-        J[c][l].re = sw ? b.re : a.re;
-        J[c][l].im = sw ? b.im : a.im;
-        J[r][l].re = sw ? a.re : b.re;
-        J[r][l].im = sw ? a.im : b.im;
-      }
-      if (sw) det = t_neg(det);
-    }
-    const cplx piv = J[c][c];
-    det = t_mul(det, piv);
-    const cplx inv = t_rdivc(1.0, piv);
-#pragma unroll
-    for (int r = c + 1; r < N; ++r) {
-      const cplx m = t_mul(J[r][c], inv);
-      const cplx mn = t_neg(m);
-#pragma unroll
-      for (int l = c + 1; l < N; ++l) J[r][l] = t_fma(mn, J[c][l], J[r][l]);
-    }
-  }
-  return det;
-}
 
 // x (real, registers) -> X = z(x) (complex) and det J per point.  sh_deform == nullptr: z = x, det = 1.
 __device__ __forceinline__ void fx_deform_points(const fx_ins *sh_deform, double lambda, double (&x)[N][P],
@@ -84,22 +46,13 @@ __device__ __forceinline__ void fx_deform_points(const fx_ins *sh_deform, double
     }
 #pragma unroll 1
   for (int p = 0; p < P; ++p) {  // one matrix at a time: 2*N*N doubles in registers
-    cplx J[N][N];
-    double zi[N];
+    double xv[N], xbv[N], zi[N];
 #pragma unroll
     for (int k = 0; k < N; ++k) {
-      const double xk = M.ld(NGH + k, p, P), xb = M.ld(NGH + N + k, p, P), gk = M.ld(k, p, P);
-      const double ls = lambda * (xk * xb);
-      zi[k] = -(ls * gk);
-#pragma unroll
-      for (int l = 0; l < N; ++l) {
-        const double h = M.ld(k <= l ? hess_slot(k, l) : hess_slot(l, k), p, P);
-        J[k][l] = cplx{0.0, -(ls * h)};
-      }
-      J[k][k].re = 1.0;
-      J[k][k].im -= lambda * (xb - xk) * gk;  // 1 - 2x = xbar - x
+      xv[k] = M.ld(NGH + k, p, P);
+      xbv[k] = M.ld(NGH + N + k, p, P);
     }
-    const cplx d = det_lu(J);
+    const cplx d = fx_jacobian_det<N>(lambda, xv, xbv, [&](int slot) { return M.ld(slot, p, P); }, zi);
 #pragma unroll
     for (int k = 0; k < N; ++k) M.st(k, p, P, zi[k]);
     M.st(NGH + 2 * N, p, P, d.re);
@@ -143,9 +96,8 @@ __global__ void __launch_bounds__(FX_THREADS) fx_integrate_cplx(const __grid_con
   const int b = blockIdx.x;
   const int chunk = b % prm.nchunks;
   const int r = (b / prm.nchunks) % prm.n_shifts;
-  const int sel_idx = b / (prm.nchunks * prm.n_shifts);
+  const int sel_idx = fx_sel_index(prm, b / (prm.nchunks * prm.n_shifts));
   const fx_sector_dev sec = prm.sectors[prm.sel[sel_idx]];
-  if (!sec.is_complex) return;
   constexpr bool vegas = RULE == FIESTA_RULE_VEGAS;
   const fx_smem_layout L = fx_layout(prm.prog_ins_max, prm.mem_doubles, N, prm.nbins, vegas);
   fx_ins *sh_prog = reinterpret_cast<fx_ins *>(smem + L.prog);
@@ -169,7 +121,8 @@ __global__ void __launch_bounds__(FX_THREADS) fx_integrate_cplx(const __grid_con
   const fx_mem<double> Mr{sh_mem + threadIdx.x, FX_THREADS};
   const fx_mem<cplx> Mc{sh_mem + threadIdx.x, FX_THREADS};
   unsigned nonfinite = 0;
-  for (uint64_t base = c0 + (uint64_t)threadIdx.x * P; base < c1; base += (uint64_t)FX_THREADS * P) {
+  for (uint64_t it = c0; it < c1; it += (uint64_t)FX_THREADS * P) {  // block-uniform trip count (see the real kernel)
+    const uint64_t base = it + (uint64_t)threadIdx.x * P;
     double x[N][P], xbar[N][P], W[P], h2[P];
     uint32_t bins[(N + 3) / 4][P];
     unsigned valid;
@@ -183,20 +136,11 @@ __global__ void __launch_bounds__(FX_THREADS) fx_integrate_cplx(const __grid_con
     IntegrateSinkCplx sink{sh_acc + threadIdx.x, Wd, valid, 0u, h2};
     fx_run<cplx, N, P>(sh_prog, X, Mc, sink);
     nonfinite += sink.nonfinite;
-    if (vegas) {
-      FX_PLOOP {
-        if ((valid >> p) & 1u) {
-#pragma unroll
-          for (int k = 0; k < N; ++k)
-            atomicAdd(sh_hist + k * prm.nbins + ((bins[k / 4][p] >> (8 * (k % 4))) & 0xffu), h2[p]);
-        }
-      }
-    }
+    if (vegas) fx_hist_points<N, P>(sh_hist, N, prm.nbins, valid, bins, h2);
   }
   __syncthreads();
-  double *out = prm.partials + (((size_t)sel_idx * prm.n_shifts + r) * prm.nchunks + chunk) * FX_ACC_SLOTS;
-  fx_block_reduce(sh_acc, sh_wsum, nslots, out);
-  fx_block_finish(prm, N, sel_idx, nonfinite, sh_hist);
+  fx_block_reduce(sh_acc, sh_wsum, nslots, fx_partial_record(prm, sel_idx, r, chunk));
+  fx_block_finish(prm, N, sel_idx, chunk, nonfinite, sh_hist);
 }
 
 struct EvalSinkCplx {
@@ -248,8 +192,9 @@ __global__ void __launch_bounds__(FX_THREADS) fx_eval_cplx(const __grid_constant
 }  // namespace
 using namespace FX_CAT(fx_cplx_n, FX_N);
 
-cudaError_t FX_CAT(fx_launch_integrate_cplx_n, FX_N)(const fx_integrate_params &prm, size_t smem, cudaStream_t st) {
-  const unsigned grid = (unsigned)((size_t)prm.nsel * prm.n_shifts * prm.nchunks);
+cudaError_t FX_CAT(fx_launch_integrate_cplx_n, FX_N)(const fx_integrate_params &prm, int nsectors, size_t smem,
+                                                     cudaStream_t st) {
+  const unsigned grid = (unsigned)((size_t)nsectors * prm.n_shifts * prm.nchunks);
   cudaError_t e;
 #define FX_LAUNCH(RULE)                                                                                                \
   {                                                                                                                    \

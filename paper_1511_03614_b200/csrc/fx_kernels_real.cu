@@ -30,15 +30,14 @@ struct IntegrateSinkReal {
 };
 
 template <int NX, int RULE>
-__global__ void __launch_bounds__(FX_THREADS, NX <= 8 ? 4 : 2) fx_integrate_real(const __grid_constant__ fx_integrate_params prm) {
+__global__ void __launch_bounds__(FX_THREADS, NX <= 4 ? 4 : NX <= 8 ? 3 : 2) fx_integrate_real(const __grid_constant__ fx_integrate_params prm) {
   constexpr int P = FX_P_REAL;
   extern __shared__ __align__(16) unsigned char smem[];
   const int b = blockIdx.x;
   const int chunk = b % prm.nchunks;
   const int r = (b / prm.nchunks) % prm.n_shifts;
-  const int sel_idx = b / (prm.nchunks * prm.n_shifts);
+  const int sel_idx = fx_sel_index(prm, b / (prm.nchunks * prm.n_shifts));
   const fx_sector_dev sec = prm.sectors[prm.sel[sel_idx]];
-  if (sec.is_complex) return;
   const int dim = prm.dim;
   constexpr bool vegas = RULE == FIESTA_RULE_VEGAS;
   const fx_smem_layout L = fx_layout(prm.prog_ins_max, prm.mem_doubles, dim, prm.nbins, vegas);
@@ -60,7 +59,10 @@ __global__ void __launch_bounds__(FX_THREADS, NX <= 8 ? 4 : 2) fx_integrate_real
   const uint64_t c1 = min(c0 + prm.chunk, prm.n_per_shift);
   const fx_mem<double> M{sh_mem + threadIdx.x, FX_THREADS};
   unsigned nonfinite = 0;
-  for (uint64_t base = c0 + (uint64_t)threadIdx.x * P; base < c1; base += (uint64_t)FX_THREADS * P) {
+  // the trip count is the same for every thread of the block (points past the end are masked by
+  // `valid`): the Vegas histogram update is a warp-collective operation
+  for (uint64_t it = c0; it < c1; it += (uint64_t)FX_THREADS * P) {
+    const uint64_t base = it + (uint64_t)threadIdx.x * P;
     double x[NX][P], xbar[NX][P], W[P], h2[P];
     uint32_t bins[(NX + 3) / 4][P];
     unsigned valid;
@@ -69,20 +71,11 @@ __global__ void __launch_bounds__(FX_THREADS, NX <= 8 ? 4 : 2) fx_integrate_real
     IntegrateSinkReal<P> sink{sh_acc + threadIdx.x, W, valid, 0u, h2};
     fx_run<double, NX, P>(sh_prog, x, M, sink);
     nonfinite += sink.nonfinite;
-    if (vegas) {
-      FX_PLOOP {
-        if ((valid >> p) & 1u) {
-#pragma unroll
-          for (int k = 0; k < NX; ++k)
-            if (k < dim) atomicAdd(sh_hist + k * prm.nbins + ((bins[k / 4][p] >> (8 * (k % 4))) & 0xffu), h2[p]);
-        }
-      }
-    }
+    if (vegas) fx_hist_points<NX, P>(sh_hist, dim, prm.nbins, valid, bins, h2);
   }
   __syncthreads();
-  double *out = prm.partials + (((size_t)sel_idx * prm.n_shifts + r) * prm.nchunks + chunk) * FX_ACC_SLOTS;
-  fx_block_reduce(sh_acc, sh_wsum, nslots, out);
-  fx_block_finish(prm, dim, sel_idx, nonfinite, sh_hist);
+  fx_block_reduce(sh_acc, sh_wsum, nslots, fx_partial_record(prm, sel_idx, r, chunk));
+  fx_block_finish(prm, dim, sel_idx, chunk, nonfinite, sh_hist);
 }
 
 template <int P>
@@ -135,11 +128,9 @@ size_t fx_integrate_smem_bytes(const fx_integrate_params &prm) {
   return fx_layout(prm.prog_ins_max, prm.mem_doubles, prm.dim, prm.nbins, prm.rule == FIESTA_RULE_VEGAS).total;
 }
 
-size_t fx_integrate_smem_bytes_native(int) { return fxj_layout().total; }
-
-cudaError_t fx_launch_integrate_real(const fx_integrate_params &prm, cudaStream_t st) {
+cudaError_t fx_launch_integrate_real(const fx_integrate_params &prm, int nsectors, cudaStream_t st) {
   const size_t smem = fx_integrate_smem_bytes(prm);
-  const unsigned grid = (unsigned)((size_t)prm.nsel * prm.n_shifts * prm.nchunks);
+  const unsigned grid = (unsigned)((size_t)nsectors * prm.n_shifts * prm.nchunks);
   cudaError_t e;
 #define FX_LAUNCH2(NX, RULE)                                                            \
   {                                                                                     \

@@ -17,6 +17,16 @@ __global__ void k_reduce_chunks(const double *partials, double *sums, int nrows,
   sums[i] = s;
 }
 
+// Vegas: the blocks' histograms of a sector, added in block order (deterministic)
+__global__ void k_reduce_hist(const double *hist_part, double *hist, int nsectors, int nchunks, int cells) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;  // sector*cells + cell
+  if (i >= (size_t)nsectors * cells) return;
+  const size_t s = i / cells, cell = i % cells;
+  double t = 0.0;
+  for (int c = 0; c < nchunks; ++c) t += hist_part[(s * nchunks + c) * cells + cell];
+  hist[i] = t;
+}
+
 // slot layout of one sums row: real sector: [k][S1,S2]; complex: [k][c][S1,S2]
 __device__ __forceinline__ int slot_of(int k, int c, int ncomp) { return (k * ncomp + c) * 2; }
 
@@ -263,10 +273,14 @@ inline unsigned blocks_for(size_t n, int t) { return (unsigned)((n + t - 1) / t)
 
 }  // namespace
 
-cudaError_t fx_launch_reduce_chunks(const double *partials, double *sums, int nsel, int R, int nchunks,
-                                    cudaStream_t st) {
-  const int nrows = nsel * R;
+cudaError_t fx_launch_reduce_chunks(const double *partials, double *sums, int nrows, int nchunks, cudaStream_t st) {
   k_reduce_chunks<<<blocks_for((size_t)nrows * FX_ACC_SLOTS, 128), 128, 0, st>>>(partials, sums, nrows, nchunks);
+  return cudaGetLastError();
+}
+
+cudaError_t fx_launch_reduce_hist(const double *hist_part, double *hist, int nsectors, int nchunks, int cells,
+                                  cudaStream_t st) {
+  k_reduce_hist<<<blocks_for((size_t)nsectors * cells, 128), 128, 0, st>>>(hist_part, hist, nsectors, nchunks, cells);
   return cudaGetLastError();
 }
 

@@ -224,7 +224,13 @@ __device__ __forceinline__ void vegas_map_coord(uint64_t t, int nbins, const dou
   uint64_t s = t >> 12;
   uint64_t prod = (2ull * s + 1ull) * (uint64_t)nbins;  // < 2^53 * NB
   bin = (int)(prod >> 53);
-  double frac = (double)(long long)(prod & ((1ull << 53) - 1ull)) * 0x1p-53;
+  // rem < 2^53 as a double, exactly and without the slow int64 -> double conversion: the high 21 and
+  // the low 32 bits become the mantissas of 2^84 + hi 2^32 and 2^52 + lo; the two offsets are taken off
+  // first (hi 2^32 - 2^52 is exact), then lo is added (hi 2^32 + lo < 2^53 is exact)
+  const uint64_t rem = prod & ((1ull << 53) - 1ull);
+  const double dhi = __hiloint2double(0x45300000, (int)(uint32_t)(rem >> 32));
+  const double dlo = __hiloint2double(0x43300000, (int)(uint32_t)rem);
+  const double frac = __dadd_rn(__dadd_rn(dhi, -(0x1p84 + 0x1p52)), dlo) * 0x1p-53;
   double lo = edges[bin];
   double width = edges[bin + 1] - lo;
   x = fma(frac, width, lo);

@@ -98,7 +98,7 @@ def test_mc_transform_is_identity(fb, ctx):
 
 # ------------------------------------------------------------------------------ A5: program walk
 
-def _eval_case(ctx, wl, nsec, npts, seed, label=None):
+def _eval_case(ctx, wl, nsec, npts, seed, label=None, tier=None):
     prog = ctx.compile(wl.sectors, wl.dim)
     rng = np.random.default_rng(seed)
     x = rng.random((npts, wl.dim))
@@ -109,24 +109,34 @@ def _eval_case(ctx, wl, nsec, npts, seed, label=None):
             x[k, k] = 1e-9
     worst = 0.0
     for si in range(nsec):
-        got = ctx.eval_points(prog, si, x)
+        got = ctx.eval_points(prog, si, x, tier=tier)
+        if tier is not None:
+            assert ctx.last_tiers() == ((1, 0) if tier == 1 else (0, 1))
         ref, mag = oracle_values_and_magnitude(spec(wl.sectors[si]), x)
         worst = max(worst, check_points(got, ref, mag, label=None if label is None else f"{label} sector {si}"))
     prog.close()
     return worst
 
 
+@pytest.mark.parametrize("tier", [1, 0])
 @pytest.mark.parametrize("name,nsec,npts", [("C1", 1, 2000), ("C2", 6, 1537), ("C3", 4, 1025), ("C4", 4, 700),
                                             ("C5", 4, 999)])
-def test_per_point_parity_configs(ctx, name, nsec, npts):
+def test_per_point_parity_configs(ctx, name, nsec, npts, tier):
+    """Per-point values of every configuration against the oracle, 1e-12 * M (R14), on BOTH forms of the
+    program: tier 1 = the native kernel (the generated program body the benchmarked integration kernels
+    are assembled from, in the eval kernel), tier 0 = the interpreter."""
     wl = make_workload(name, nsectors=nsec, npoints=1 << 12)
-    assert _eval_case(ctx, wl, nsec, npts, 11, label=f"per-point {name}") <= 1.0
+    label = f"per-point {name} {'native' if tier else 'interpreter'}"
+    assert _eval_case(ctx, wl, nsec, npts, 11, label=label, tier=tier) <= 1.0
 
 
 @pytest.mark.parametrize("npts", [1, 3, 511, 512, 513])
 def test_per_point_ragged_counts(ctx, npts):
     wl = make_workload("C2", nsectors=1, npoints=1 << 12)
-    assert _eval_case(ctx, wl, 1, npts, npts) <= 1.0
+    assert _eval_case(ctx, wl, 1, npts, npts, tier=1) <= 1.0
+    assert _eval_case(ctx, wl, 1, npts, npts, tier=0) <= 1.0
+    wl = make_workload("C4", nsectors=1, npoints=1 << 12)
+    assert _eval_case(ctx, wl, 1, npts, npts, tier=1) <= 1.0
 
 
 def test_eval_zero_points(ctx):
@@ -162,38 +172,87 @@ def test_lattice_partial_sums_parity(fb, ctx, name, nsec, npts, nsh):
 
 
 @pytest.mark.parametrize("name,nsec,npts,nsh", [("C1", 1, 1 << 16, 8), ("C2", 3, 1 << 15, 1), ("C3", 2, 1 << 15, 8),
-                                                ("C5", 2, 1 << 13, 2), ("C3", 1, 64, 1), ("C2", 2, 8 * 256, 8)])
-def test_native_and_interpreter_tiers_agree_bitwise(fb, ctx, monkeypatch, name, nsec, npts, nsh):
-    """fiesta_compile's two forms of a real sector's program (interpreted fx_ins walk; the same
-    sequence assembled to a native kernel) do the same operations in the same order: every partial
-    sum and every result is bit-identical, and the interpreter tier on its own meets the oracle."""
+                                                ("C5", 2, 1 << 13, 2), ("C3", 1, 64, 1), ("C2", 2, 8 * 256, 8),
+                                                ("C4", 2, 1 << 13, 2)])
+def test_native_and_interpreter_tiers_agree_bitwise(fb, ctx, name, nsec, npts, nsh):
+    """fiesta_compile's two forms of a sector's program (interpreted fx_ins walk; the same sequence
+    assembled to a native kernel) do the same operations in the same order: every partial sum and
+    every result is bit-identical, and the interpreter tier on its own meets the oracle.  This is
+    what lets fiesta_integrate serve a sector with whichever form is ready."""
     wl = make_workload(name, nsectors=nsec, npoints=npts, n_shifts=nsh)
-    rule = fb.Rule(kind=fb.RULE_LATTICE, n_shifts=nsh, korobov_a=wl.korobov_a or 1129, periodize_r=3)
-    monkeypatch.setenv("FIESTA_JIT", "0")
-    prog_i = ctx.compile(wl.sectors, wl.dim)
-    monkeypatch.setenv("FIESTA_JIT", "1")
-    prog_n = ctx.compile(wl.sectors, wl.dim)
+    rule = fb.Rule(kind=fb.RULE_LATTICE, n_shifts=nsh, korobov_a=wl.korobov_a if wl.rule == fb.RULE_LATTICE else 1129,
+                   periodize_r=3)
+    prog = ctx.compile(wl.sectors, wl.dim)
+    a = ctx.partial_sums(prog, npts, rule, wl.seed, tier=fb.TIER_INTERPRETER)
+    assert ctx.last_tiers() == (0, nsec)
+    b = ctx.partial_sums(prog, npts, rule, wl.seed, tier=fb.TIER_NATIVE)
+    assert ctx.last_tiers() == (nsec, 0)
     for si in range(nsec):
-        assert prog_i.native(si) == (False, "")
-        assert prog_n.native(si) == (True, ""), prog_n.native(si)
-    a = ctx.partial_sums(prog_i, npts, rule, wl.seed)
-    b = ctx.partial_sums(prog_n, npts, rule, wl.seed)
+        ok, info = prog.native(si, fb.RULE_LATTICE)
+        assert ok and "Used" in info, info
     assert a.tobytes() == b.tobytes()
-    ra = ctx.integrate(prog_i, npts, rule, wl.seed)
-    rb = ctx.integrate(prog_n, npts, rule, wl.seed)
+    ra = ctx.integrate(prog, npts, rule, wl.seed, tier=fb.TIER_INTERPRETER)
+    rb = ctx.integrate(prog, npts, rule, wl.seed, tier=fb.TIER_NATIVE)
     assert ra.tobytes() == rb.tobytes()
+    assert ctx.integrate(prog, npts, rule, wl.seed).tobytes() == ra.tobytes()      # whichever is ready
     gv = OP.korobov_genvec(rule.korobov_a, npts // nsh, wl.dim)
     s1, s2, sa = OI.lattice_partial_sums(spec(wl.sectors[0]), npts // nsh, nsh, gv, 3, wl.seed)
     check_sums(a[0], s1, s2, sa)
     # a selection that mixes the order, and a sector list of one
     sel = list(range(nsec))[::-1]
-    assert ctx.partial_sums(prog_n, npts, rule, wl.seed, sectors=sel).tobytes() == a[sel].tobytes()
+    assert ctx.partial_sums(prog, npts, rule, wl.seed, sectors=sel, tier=fb.TIER_NATIVE).tobytes() == a[sel].tobytes()
+    # plain MC and one Vegas iteration: the other two native kernels of the same sectors
+    mc = fb.Rule(kind=fb.RULE_MC)
+    a = ctx.partial_sums(prog, 5000, mc, 3, tier=fb.TIER_INTERPRETER)
+    b = ctx.partial_sums(prog, 5000, mc, 3, tier=fb.TIER_NATIVE)
+    assert ctx.last_tiers() == (nsec, 0) and a.tobytes() == b.tobytes()
+    vr = fb.Rule(kind=fb.RULE_VEGAS, vegas_bins=37, vegas_iters=1)
+    grid = np.sort(np.random.default_rng(1).random((wl.dim, 38)), axis=1)
+    grid[:, 0], grid[:, -1] = 0.0, 1.0
+    sa_, ha = ctx.vegas_iteration(prog, nsec - 1, 3001, vr, 9, 2, grid, tier=fb.TIER_INTERPRETER)
+    sb_, hb = ctx.vegas_iteration(prog, nsec - 1, 3001, vr, 9, 2, grid, tier=fb.TIER_NATIVE)
+    assert ctx.last_tiers() == (1, 0)
+    assert sa_.tobytes() == sb_.tobytes() and ha.tobytes() == hb.tobytes()
+    # a full Vegas run is reproducible bit for bit, on either tier (no atomics anywhere in the histogram)
+    vr3 = fb.Rule(kind=fb.RULE_VEGAS, vegas_bins=20, vegas_iters=3)
+    r1 = ctx.integrate(prog, 4096, vr3, 5, tier=fb.TIER_INTERPRETER, allow_nonfinite=True)
+    r2 = ctx.integrate(prog, 4096, vr3, 5, tier=fb.TIER_NATIVE, allow_nonfinite=True)
+    r3 = ctx.integrate(prog, 4096, vr3, 5, tier=fb.TIER_NATIVE, allow_nonfinite=True)
+    assert r1.tobytes() == r2.tobytes() == r3.tobytes()
 
 
-def test_complex_sectors_stay_on_the_interpreter(fb, ctx):
-    wl = make_workload("C4", nsectors=1, npoints=1 << 12)
+def test_native_tier_is_off_with_fiesta_jit_0(fb, ctx, monkeypatch):
+    wl = make_workload("C2", nsectors=2, npoints=1 << 12)
+    monkeypatch.setenv("FIESTA_JIT", "0")
     prog = ctx.compile(wl.sectors, wl.dim)
-    assert prog.native(0) == (False, "")
+    monkeypatch.delenv("FIESTA_JIT")
+    assert prog.wait_native() == 0 and prog.native(0) == (False, "")
+    rule = fb.Rule.from_workload(wl)
+    ctx.integrate(prog, wl.npoints, rule, wl.seed)
+    assert ctx.last_tiers() == (0, 2)
+    with pytest.raises(fb.FiestaError):
+        ctx.eval_points(prog, 0, np.full((3, wl.dim), 0.5), tier=fb.TIER_NATIVE)
+
+
+def test_mixed_real_and_complex_call(fb, ctx):
+    """One fiesta_integrate call over real and complex sectors (same K): each kind on its own kernels,
+    results in selection order, equal to the separate calls, on every tier."""
+    wr = make_workload("C2", nsectors=2, npoints=1 << 12)           # dim 6, K = 4, real
+    s = wr.sectors[1]
+    cplx = SectorText(77, s.texts, is_complex=True, deform_f_index=2, lam=0.3)
+    prog = ctx.compile([wr.sectors[0], cplx, wr.sectors[1]], wr.dim)
+    rule = fb.Rule(kind=fb.RULE_LATTICE, n_shifts=2, korobov_a=wr.korobov_a, periodize_r=3)
+    for tier in (fb.TIER_INTERPRETER, fb.TIER_NATIVE, None):
+        res = ctx.integrate(prog, 1 << 12, rule, 5, tier=tier)
+        for i in range(3):
+            one = ctx.integrate(prog, 1 << 12, rule, 5, sectors=[i], tier=tier)
+            assert one.tobytes() == res[i:i + 1].tobytes()
+        assert np.all(res[0]["im"] == 0) and np.all(res[2]["im"] == 0) and np.all(res[1]["im_err"] > 0)
+    sec = SectorSpec(cplx.texts, 77, True, 2, 0.3)
+    gv = OP.korobov_genvec(wr.korobov_a, 1 << 11, wr.dim)
+    val, sig = OI.integrate_lattice(sec, 1 << 12, 2, gv, 3, 5)
+    assert np.allclose(res[1]["re"], np.asarray(val, dtype=float)[:, 0], rtol=1e-9)
+    assert np.allclose(res[1]["im"], np.asarray(val, dtype=float)[:, 1], rtol=1e-9, atol=1e-12 * np.abs(np.asarray(val, dtype=float)).max())
 
 
 def test_sector_selection_and_order(fb, ctx):
