@@ -924,7 +924,11 @@ namespace {
 bool in_fam(int op, int base, int n) { return op >= base && op < base + n; }
 }
 
-void fill_info(const std::vector<fx_ins> &code, fiesta_compile_info &info) {
+// FP64 flops of a program, counted as fma 2, mul/add 1, division 15, log/exp 40 (nominal weights for
+// the library routines).  Complex programs (cplx): every instruction by the real operations of its
+// handler (gen_interp_ptx.py): complex*complex 6, complex fma 8, fma with a real immediate 7 or 4,
+// complex +- 2, division 6 + 15 + ..., log = log + atan2 (80), exp = exp + sincos (80).
+void fill_info(const std::vector<fx_ins> &code, fiesta_compile_info &info, bool cplx) {
   for (auto &i : code) {
     int op = i.op;
     if (op == FX_END) continue;
@@ -937,20 +941,33 @@ void fill_info(const std::vector<fx_ins> &code, fiesta_compile_info &info) {
     info.n_fp64_ops++;
     if (fma) {
       info.n_fma++;
-      info.flops += 2;
+      if (!cplx) info.flops += 2;
+      else if (in_fam(op, FX_FMA_RC_A, FX_LR) || in_fam(op, FX_FMA_MC_A, FX_L)) info.flops += 4;  // r*imm + a: 2 fma
+      else if (in_fam(op, FX_FMA_AR_C, FX_LR) || in_fam(op, FX_FMA_AM_C, FX_L)) info.flops += 7;  // a*b + imm: 3 fma + mul
+      else info.flops += 8;                                                                       // a*b + c: 4 fma
     } else if (div) {
       info.n_div++;
-      info.flops += 15;
+      if (!cplx) info.flops += 15;
+      else if (op == FX_DIVC) info.flops += 30;
+      else if (op == FX_RDIVC) info.flops += 3 + 15 + 2;
+      else info.flops += 3 + 15 + 6 + 2;
     } else if (op == FX_LOG) {
       info.n_log++;
-      info.flops += 40;
+      info.flops += cplx ? 80 : 40;
     } else if (op == FX_EXP) {
       info.n_exp++;
-      info.flops += 40;
+      info.flops += cplx ? 80 : 40;
     } else if (op == FX_SQRT) {
-      info.flops += 15;
-    } else
+      info.flops += cplx ? 40 : 15;
+    } else if (!cplx) {
       info.flops += 1;
+    } else if (in_fam(op, FX_MUL_R, FX_LR) || in_fam(op, FX_MUL_UP, FX_L) || in_fam(op, FX_MULM, FX_L) || op == FX_SQR) {
+      info.flops += 6;  // complex * complex: 2 mul + 2 fma
+    } else if (in_fam(op, FX_ADDC, FX_L) || op == FX_RSUBC) {
+      info.flops += 1;  // real immediate added to the real part
+    } else {
+      info.flops += 2;  // componentwise: complex +-, times a real immediate
+    }
   }
 }
 
@@ -1076,7 +1093,7 @@ CompiledSector compile_sector(const char *const *texts, int K, int dim, bool is_
     cs.info.n_reg_temps = em.s_high;
     cs.info.n_mem_slots = em.mhigh;
   }
-  fill_info(cs.main, cs.info);
+  fill_info(cs.main, cs.info, cs.is_complex);
 
   if (cs.deform_on) {
     if (deform_f_index > (int)funcs0.size())
@@ -1104,7 +1121,7 @@ CompiledSector compile_sector(const char *const *texts, int K, int dim, bool is_
     cs.n_mem_deform = em.mhigh;
     cs.info.n_deform_ops = (int)cs.deform.size() - 1;
     fiesta_compile_info di{};
-    fill_info(cs.deform, di);
+    fill_info(cs.deform, di, false);
     cs.info.flops += di.flops;
   }
   return cs;

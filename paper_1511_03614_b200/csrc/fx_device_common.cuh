@@ -72,7 +72,7 @@ struct fx_tP {
   uint64_t t[P];
 };
 template <int P>
-static __device__ __noinline__ fx_coordP<P> fx_lattice_coord(fx_tP<P> t, const fx_transform *tf /* shared memory */) {
+__device__ __forceinline__ fx_coordP<P> fx_lattice_coord_body(fx_tP<P> t, const fx_transform *tf /* shared memory */) {
   fx_coordP<P> c;
   if (tf->r == 3) {  // the default weight: no switch
 #pragma unroll
@@ -84,26 +84,41 @@ static __device__ __noinline__ fx_coordP<P> fx_lattice_coord(fx_tP<P> t, const f
   return c;
 }
 
-static __device__ __noinline__ fx_tpair fx_philox_pair(uint64_t seed, uint32_t sector_id, uint32_t tag, uint32_t it, uint64_t j,
-                                                uint32_t kb) {
+template <int P>
+static __device__ __noinline__ fx_coordP<P> fx_lattice_coord(fx_tP<P> t, const fx_transform *tf) {
+  return fx_lattice_coord_body<P>(t, tf);
+}
+
+__device__ __forceinline__ fx_tpair fx_philox_pair_body(uint64_t seed, uint32_t sector_id, uint32_t tag, uint32_t it,
+                                                        uint64_t j, uint32_t kb) {
   fx_tpair r;
   philox_t_pair(seed, sector_id, tag, it, j, kb, r.e, r.o);
   return r;
+}
+static __device__ __noinline__ fx_tpair fx_philox_pair(uint64_t seed, uint32_t sector_id, uint32_t tag, uint32_t it, uint64_t j,
+                                                uint32_t kb) {
+  return fx_philox_pair_body(seed, sector_id, tag, it, j, kb);
 }
 
 struct fx_vcoord {
   double x, w;
   int bin;
 };
-static __device__ __noinline__ fx_vcoord fx_vegas_coord(uint64_t t, int nbins, const double *edges) {
+__device__ __forceinline__ fx_vcoord fx_vegas_coord_body(uint64_t t, int nbins, const double *edges) {
   fx_vcoord c;
   vegas_map_coord(t, nbins, edges, c.x, c.w, c.bin);
   return c;
 }
+static __device__ __noinline__ fx_vcoord fx_vegas_coord(uint64_t t, int nbins, const double *edges) {
+  return fx_vegas_coord_body(t, nbins, edges);
+}
 
 // Points j0..j0+P-1 of (sector, shift r / iteration) -> real x, xbar = 1-x, weight W, Vegas bins.
-// RULE is a compile-time constant: each rule has its own kernel instantiation.
-template <int RULE, int NX, int P>
+// RULE is a compile-time constant: each rule has its own kernel instantiation.  INL: the per-coordinate
+// helpers inline instead of out of line -- an out-of-line call makes the kernel save the values it
+// has live across the call to local memory, which the kernels with many such values (Vegas with 4
+// points per thread; all complex kernels) avoid this way at the price of longer code.
+template <int RULE, int NX, int P, bool INL = false>
 __device__ __forceinline__ void fx_make_points(const fx_integrate_params &prm, int dim, uint32_t sector_id,
                                                const uint64_t *sh_delta, const double *sh_grid, uint64_t j0,
                                                uint64_t jend, double (&x)[NX][P], double (&xbar)[NX][P],
@@ -124,7 +139,7 @@ __device__ __forceinline__ void fx_make_points(const fx_integrate_params &prm, i
         const uint64_t G = fx_lattice_steps(sh_delta)[k];
         fx_tP<P> tt;
         FX_PLOOP { tt.t[p] = (j0 + p) * G + sh_delta[k]; }
-        const fx_coordP<P> c = fx_lattice_coord<P>(tt, tf);
+        const fx_coordP<P> c = INL ? fx_lattice_coord_body<P>(tt, tf) : fx_lattice_coord<P>(tt, tf);
         FX_PLOOP {
           x[k][p] = c.x[p];
           xbar[k][p] = c.xbar[p];
@@ -143,7 +158,9 @@ __device__ __forceinline__ void fx_make_points(const fx_integrate_params &prm, i
     for (int kb = 0; kb < (NX + 1) / 2; ++kb) {
       FX_PLOOP {
         fx_tpair tp{0ull, 0ull};
-        if (2 * kb < dim) tp = fx_philox_pair(prm.seed, sector_id, FX_TAG_MC, (uint32_t)prm.iteration, j0 + p, kb);
+        if (2 * kb < dim)
+          tp = INL ? fx_philox_pair_body(prm.seed, sector_id, FX_TAG_MC, (uint32_t)prm.iteration, j0 + p, kb)
+                   : fx_philox_pair(prm.seed, sector_id, FX_TAG_MC, (uint32_t)prm.iteration, j0 + p, kb);
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
           const int k = 2 * kb + h;
@@ -151,7 +168,8 @@ __device__ __forceinline__ void fx_make_points(const fx_integrate_params &prm, i
             const uint64_t t = h ? tp.o : tp.e;
             if (k < dim) {
               if constexpr (RULE == FIESTA_RULE_VEGAS) {
-                const fx_vcoord c = fx_vegas_coord(t, prm.nbins, sh_grid + k * (prm.nbins + 1));
+                const double *edges = sh_grid + k * (prm.nbins + 1);
+                const fx_vcoord c = INL ? fx_vegas_coord_body(t, prm.nbins, edges) : fx_vegas_coord(t, prm.nbins, edges);
                 x[k][p] = c.x;
                 xbar[k][p] = 1.0 - c.x;
                 W[p] *= c.w;

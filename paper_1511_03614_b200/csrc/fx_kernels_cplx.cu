@@ -126,7 +126,7 @@ __global__ void __launch_bounds__(FX_THREADS) fx_integrate_cplx(const __grid_con
     double x[N][P], xbar[N][P], W[P], h2[P];
     uint32_t bins[(N + 3) / 4][P];
     unsigned valid;
-    fx_make_points<RULE, N, P>(prm, N, (uint32_t)sec.sector_id, sh_delta, sh_grid, base, c1, x, xbar, W, valid, bins);
+    fx_make_points<RULE, N, P, true>(prm, N, (uint32_t)sec.sector_id, sh_delta, sh_grid, base, c1, x, xbar, W, valid, bins);
     cplx X[N][P], Wd[P];
     fx_deform_points(sh_deform, sec.lambda, x, xbar, Mr, X, Wd);
     FX_PLOOP {

@@ -66,7 +66,7 @@ __global__ void __launch_bounds__(FX_THREADS, NX <= 4 ? 4 : NX <= 8 ? 3 : 2) fx_
     double x[NX][P], xbar[NX][P], W[P], h2[P];
     uint32_t bins[(NX + 3) / 4][P];
     unsigned valid;
-    fx_make_points<RULE, NX, P>(prm, dim, (uint32_t)sec.sector_id, sh_delta, sh_grid, base, c1, x, xbar, W, valid, bins);
+    fx_make_points<RULE, NX, P, RULE == FIESTA_RULE_VEGAS>(prm, dim, (uint32_t)sec.sector_id, sh_delta, sh_grid, base, c1, x, xbar, W, valid, bins);
     FX_PLOOP { h2[p] = 0.0; }
     IntegrateSinkReal<P> sink{sh_acc + threadIdx.x, W, valid, 0u, h2};
     fx_run<double, NX, P>(sh_prog, x, M, sink);
