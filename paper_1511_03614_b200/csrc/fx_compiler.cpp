@@ -28,6 +28,10 @@
 namespace fx {
 namespace {
 
+#ifndef FX_HORNER_LOOK
+#define FX_HORNER_LOOK 1
+#endif
+
 [[noreturn]] void fail(int code, const std::string &msg) { throw CompileError{code, msg}; }
 
 // ------------------------------------------------------------------------------ raw DAG
@@ -821,7 +825,84 @@ struct Emitter {
     for (int a : atoms) consume(a);
   }
 
-  // Greedy multivariate Horner: p = v*q + r with v the atom that divides most terms.
+  // p = v*q + r
+  static void split(const Poly &terms, int v, Poly &q, Poly &r) {
+    for (auto &t : terms) {
+      bool has = false;
+      Term u;
+      u.c = t.c;
+      for (auto &fe : t.f) {
+        if (fe.first == v) {
+          has = true;
+          if (fe.second > 1) u.f.push_back({fe.first, fe.second - 1});
+        } else
+          u.f.push_back(fe);
+      }
+      (has ? q : r).push_back(u);
+    }
+  }
+  static int most_frequent(const Poly &terms) {
+    std::map<int, int> cnt;
+    for (auto &t : terms)
+      for (auto &fe : t.f) cnt[fe.first]++;
+    int v = -1, best = 0;
+    for (auto &kv : cnt)
+      if (kv.second > best) {
+        best = kv.second;
+        v = kv.first;
+      }
+    return v;
+  }
+  // FP64-pipe cost of what horner() emits for `terms`, in issue slots of the native tier: a multiply
+  // or an FMA with two register operands 1, an FMA that reads three registers (the fold A[d] =
+  // A[d+1]*v + A[d]) 1.5 -- a three-operand DFMA issues at 2/3 rate on sm_100a.
+  // `v` >= 0: factor out v at this node.  Below (and here if v < 0): the best of all atoms for `look`
+  // more levels, then the greedy rule (the atom dividing most terms).
+  static double cost(const Poly &terms, int v, int look) {
+    if (terms.empty()) return 0.0;
+    if (terms.size() == 1) {
+      int nf = 0;
+      for (auto &fe : terms[0].f) nf += fe.second;
+      return (double)nf;
+    }
+    if (v < 0) {
+      if (look <= 0 || terms.size() <= 2) v = most_frequent(terms);
+      else return best_variable(terms, look).second;
+    }
+    Poly q, r;
+    split(terms, v, q, r);
+    const int lk = look - 1;
+    if (r.empty()) return cost(q, -1, lk) + 1.0;
+    const bool q_const = q.size() == 1 && q[0].f.empty();
+    const bool r_const = r.size() == 1 && r[0].f.empty();
+    if (q_const) return cost(r, -1, lk) + 1.0;
+    if (r_const) return cost(q, -1, lk) + 1.0;
+    if (r.size() == 1 && r[0].f.size() == 1 && r[0].f[0].second == 1) return cost(q, -1, lk) + 2.0;
+    if (q.size() == 1) return cost(r, -1, lk) + cost(q, -1, 0) + 1.0;  // monomial q: muls, then the fold with an immediate
+    return cost(r, -1, lk) + cost(q, -1, lk) + 1.5;
+  }
+  // every atom that divides at least two terms is tried as the variable to factor out
+  static std::pair<int, double> best_variable(const Poly &terms, int look) {
+    std::map<int, int> cnt;
+    for (auto &t : terms)
+      for (auto &fe : t.f) cnt[fe.first]++;
+    int best_v = -1, best_n = 0;
+    double best_c = 0.0;
+    for (auto &kv : cnt) {
+      if (kv.second < 2 && best_v >= 0 && best_n >= 2) continue;
+      const double c = cost(terms, kv.first, look);
+      if (best_v < 0 || c < best_c - 1e-9 || (c < best_c + 1e-9 && kv.second > best_n)) {
+        best_v = kv.first;
+        best_c = c;
+        best_n = kv.second;
+      }
+    }
+    return {best_v, best_c};
+  }
+  // FX_HORNER_LOOK levels of look-ahead over the greedy rule at every node that is emitted
+  static int choose_variable(const Poly &terms) { return best_variable(terms, FX_HORNER_LOOK).first; }
+
+  // Multivariate Horner: p = v*q + r, v chosen by choose_variable.
   void horner(const Poly &terms) {
     if (terms.empty()) {
       ins(FX_LDC + lvl, 0, 0.0);
@@ -846,29 +927,9 @@ struct Emitter {
       }
       return;
     }
-    std::map<int, int> cnt;
-    for (auto &t : terms)
-      for (auto &fe : t.f) cnt[fe.first]++;
-    int v = -1, best = 0;
-    for (auto &kv : cnt)
-      if (kv.second > best) {
-        best = kv.second;
-        v = kv.first;
-      }
+    const int v = choose_variable(terms);
     Poly q, r;
-    for (auto &t : terms) {
-      bool has = false;
-      Term u;
-      u.c = t.c;
-      for (auto &fe : t.f) {
-        if (fe.first == v) {
-          has = true;
-          if (fe.second > 1) u.f.push_back({fe.first, fe.second - 1});
-        } else
-          u.f.push_back(fe);
-      }
-      (has ? q : r).push_back(u);
-    }
+    split(terms, v, q, r);
     Opnd vo = operand_of(v);
     if (r.empty()) {
       horner(q);
@@ -899,6 +960,27 @@ struct Emitter {
     // general case p = q*v + r: r stays in A[lvl] while q is evaluated one level up, then one
     // FMA folds them -- no store/reload of the partial result
     horner(r);
+    if (lvl + 1 < FX_L && q.size() == 1) {
+      // q = c*m, one monomial: the product m*v WITHOUT its coefficient, which enters at the fold as
+      // the immediate of A[d] = A[d+1]*c + A[d] -- two register operands where the fold through
+      // FMA_UP reads three (a three-operand DFMA issues at 2/3 rate on sm_100a)
+      ++lvl;
+      bool started = false;
+      for (auto &fe : q[0].f) {
+        Opnd o = operand_of(fe.first);
+        for (int e = 0; e < fe.second; ++e) {
+          if (!started) {
+            mulc_load(o, 1.0);
+            started = true;
+          } else
+            mul(o);
+        }
+      }
+      mul(vo);
+      --lvl;
+      ins(FX_FMA_UPC + lvl, 0, q[0].c);
+      return;
+    }
     if (lvl + 1 < FX_L) {
       ++lvl;
       horner(q);
@@ -933,7 +1015,7 @@ void fill_info(const std::vector<fx_ins> &code, fiesta_compile_info &info, bool 
     int op = i.op;
     if (op == FX_END) continue;
     info.n_ir_ops++;
-    bool fma = in_fam(op, FX_FMA_AR_C, 3 * FX_LR) || in_fam(op, FX_FMA_AR_M, FX_LR) || in_fam(op, FX_FMA_MC_A, 2 * FX_L);
+    bool fma = in_fam(op, FX_FMA_AR_C, 3 * FX_LR) || in_fam(op, FX_FMA_AR_M, FX_LR) || in_fam(op, FX_FMA_MC_A, 3 * FX_L);
     bool div = in_fam(op, FX_DIV_R, 2 * FX_NR) || op == FX_DIVC || op == FX_RDIVC || op == FX_DIVM || op == FX_RDIVM;
     bool move = in_fam(op, FX_LD_R, FX_LR) || in_fam(op, FX_ST_S, FX_NS) || in_fam(op, FX_LDC, FX_L) ||
                 in_fam(op, FX_LDM, 2 * FX_L) || op == FX_OUT || op == FX_NEG;
@@ -942,7 +1024,7 @@ void fill_info(const std::vector<fx_ins> &code, fiesta_compile_info &info, bool 
     if (fma) {
       info.n_fma++;
       if (!cplx) info.flops += 2;
-      else if (in_fam(op, FX_FMA_RC_A, FX_LR) || in_fam(op, FX_FMA_MC_A, FX_L)) info.flops += 4;  // r*imm + a: 2 fma
+      else if (in_fam(op, FX_FMA_RC_A, FX_LR) || in_fam(op, FX_FMA_MC_A, FX_L) || in_fam(op, FX_FMA_UPC, FX_L)) info.flops += 4;  // r*imm + a: 2 fma
       else if (in_fam(op, FX_FMA_AR_C, FX_LR) || in_fam(op, FX_FMA_AM_C, FX_L)) info.flops += 7;  // a*b + imm: 3 fma + mul
       else info.flops += 8;                                                                       // a*b + c: 4 fma
     } else if (div) {
@@ -1131,7 +1213,7 @@ std::string disassemble(const std::vector<fx_ins> &prog) {
   static const char *lr[] = {"A%d=%3$g*R%2$d", "A%d*=R%d", "A%d=A%1$d*R%d+%g", "A%d+=R%d*%g", "A%d+=A[+1]*R%d",
                              "A%d+=R%d", "A%d=R%d", "A%d=A%1$d*R%d+M"};
   static const char *lv[] = {"A%d=imm", "A%d+=imm", "A%d*=imm", "A%d+=A[+1]", "A%d*=A[+1]", "A%d=M", "M=A%d",
-                             "A%d+=M", "A%d*=M", "A%d+=M*imm", "A%d=A%1$d*M+imm"};
+                             "A%d+=M", "A%d*=M", "A%d+=M*imm", "A%d=A%1$d*M+imm", "A%d+=A[+1]*imm"};
   static const char *r0[] = {"A-=R%d", "A=R%d-A", "A/=R%d", "A=R%d/A"};
   static const char *single[] = {"A=imm-A", "A/=imm", "A=imm/A", "A-=M", "A=M-A", "A/=M", "A=M/A", "A=-A", "A=A*A",
                                  "A=log A", "A=exp A", "A=sqrt A", "OUT", "END"};

@@ -50,6 +50,19 @@ __device__ __forceinline__ uint64_t *fx_lattice_steps(uint64_t *sh_delta) {
 __device__ __forceinline__ const uint64_t *fx_lattice_steps(const uint64_t *sh_delta) {
   return sh_delta + FX_NXMAX + 80 / 8;
 }
+// ... and behind them the block's point range [c0, c1) and its pass count (native kernels): read back
+// through volatile loads in every pass, so that they are not held in registers across the program body
+__device__ __forceinline__ uint64_t *fx_block_range(uint64_t *sh_delta) { return sh_delta + FX_NXMAX + 80 / 8 + FX_NXMAX; }
+__device__ __forceinline__ uint64_t fx_lds_volatile(const uint64_t *p) {
+  uint64_t v;
+  asm volatile("ld.volatile.shared.u64 %0, [%1];" : "=l"(v) : "r"((uint32_t)__cvta_generic_to_shared(p)));
+  return v;
+}
+__device__ __forceinline__ unsigned fx_tid_volatile() {
+  unsigned t;
+  asm volatile("mov.u32 %0, %%tid.x;" : "=r"(t));
+  return t;
+}
 
 // Out-of-line helpers: the evaluation kernels call them once per coordinate.  Keeping one copy of
 // each (instead of NX*P inlined copies) keeps the per-batch code outside the program walk small, so
@@ -220,27 +233,34 @@ __device__ __forceinline__ void fx_block_setup(const fx_integrate_params &prm, i
 }
 
 // Vegas histogram (R8): h[k][bin] += v for one point per lane, into the
-// WARP's own histogram in shared memory.  Warp-aggregated: lanes whose points fall into the same bin
-// are found with match.any and their values are added in lane order by every lane of the group; the
-// group's first lane then does one plain read-modify-write.  No atomics, and the order of every
-// addition is fixed, so the histogram -- like the sums -- is bit-reproducible.
+// WARP's own histogram in shared memory.  Warp-aggregated: the lanes whose points fall into the
+// same bin of dimension k are found with match.any; each group is a linked list in lane order
+// (next = the next higher lane of the group), and its values are added by pointer jumping -- every
+// lane adds the value of its successor and then points to its successor's successor, so after
+// ceil(log2(group size)) steps the group's first lane holds the group's sum, in a summation tree
+// fixed by the lanes' positions alone; that lane then does one plain read-modify-write.  No atomics,
+// every addition in a fixed order: the histogram -- like the sums -- is bit-reproducible.
+__device__ __forceinline__ unsigned fx_hist_peers(unsigned bin, bool valid) {
+  const unsigned lane = threadIdx.x & 31u;
+  return __match_any_sync(0xffffffffu, valid ? bin : (0x100u | lane));  // a point past the end matches nobody
+}
 __device__ __forceinline__ void fx_hist_add(double *warp_hist_k /* this warp's h[k][0..nbins) */, unsigned bin,
-                                            double v, bool valid) {
+                                            unsigned peers, double v, bool valid) {
   const unsigned full = 0xffffffffu;
   const unsigned lane = threadIdx.x & 31u;
-  const unsigned key = valid ? bin : (0x100u | lane);  // a point past the end matches nobody
-  const unsigned peers = __match_any_sync(full, key);
-  const unsigned maxn = __reduce_max_sync(full, (unsigned)__popc(peers));
-  double sum = 0.0;
-  unsigned m = peers;
-  for (unsigned it = 0; it < maxn; ++it) {
-    const int src = m ? (__ffs(m) - 1) : (int)lane;
+  const unsigned below = (1u << lane) - 1u;
+  const unsigned higher = peers & ~(below | (1u << lane));
+  int nxt = higher ? (__ffs(higher) - 1) : -1;
+  while (__any_sync(full, nxt >= 0)) {
+    const int src = nxt >= 0 ? nxt : (int)lane;
     const double t = __shfl_sync(full, v, src);
-    if (m) sum += t;
-    m &= m - 1;
+    const int n2 = __shfl_sync(full, nxt, src);
+    if (nxt >= 0) {
+      v += t;
+      nxt = n2;
+    }
   }
-  if (valid && lane == (unsigned)(__ffs(peers) - 1)) warp_hist_k[bin] += sum;
-  __syncwarp();
+  if (valid && (peers & below) == 0u) warp_hist_k[bin] += v;
 }
 
 // all dimensions of the P points of a thread, point by point (the order both tiers use)
@@ -249,9 +269,15 @@ __device__ __forceinline__ void fx_hist_points(double *sh_hist, int dim, int nbi
                                                const uint32_t (&bins)[(NX + 3) / 4][P], const double (&h2)[P]) {
   double *wh = sh_hist + (size_t)(threadIdx.x >> 5) * dim * nbins;
   FX_PLOOP {
+    const bool ok = (valid >> p) & 1u;
+    unsigned peers[NX];  // all matches first: their latencies overlap
 #pragma unroll
     for (int k = 0; k < NX; ++k)
-      if (k < dim) fx_hist_add(wh + k * nbins, (bins[k / 4][p] >> (8 * (k % 4))) & 0xffu, h2[p], (valid >> p) & 1u);
+      if (k < dim) peers[k] = fx_hist_peers((bins[k / 4][p] >> (8 * (k % 4))) & 0xffu, ok);
+#pragma unroll
+    for (int k = 0; k < NX; ++k)
+      if (k < dim) fx_hist_add(wh + k * nbins, (bins[k / 4][p] >> (8 * (k % 4))) & 0xffu, peers[k], h2[p], ok);
+    __syncwarp();  // the next point's read-modify-writes (other lanes, same cells) come after these
   }
 }
 

@@ -57,9 +57,12 @@ template <typename T, int P>
 struct fx_vec {
   T v[P];
 };
+#ifndef FX_SLOW_ATTR  // a translation unit may ask for inline copies (see fx_kernels_cplx.cu)
+#define FX_SLOW_ATTR __noinline__
+#endif
 #define FX_SLOW_UNARY(name, fn)                                                  \
   template <typename T, int P>                                                   \
-  static __device__ __noinline__ fx_vec<T, P> name(fx_vec<T, P> a) {             \
+  static __device__ FX_SLOW_ATTR fx_vec<T, P> name(fx_vec<T, P> a) {             \
     _Pragma("unroll") for (int p = 0; p < P; ++p) a.v[p] = fn(a.v[p]);           \
     return a;                                                                    \
   }
@@ -67,7 +70,7 @@ FX_SLOW_UNARY(fx_slow_log, t_log)
 FX_SLOW_UNARY(fx_slow_exp, t_exp)
 FX_SLOW_UNARY(fx_slow_sqrt, t_sqrt)
 template <typename T, int P>
-static __device__ __noinline__ fx_vec<T, P> fx_slow_div(fx_vec<T, P> a, fx_vec<T, P> b) {
+static __device__ FX_SLOW_ATTR fx_vec<T, P> fx_slow_div(fx_vec<T, P> a, fx_vec<T, P> b) {
 #pragma unroll
   for (int p = 0; p < P; ++p) a.v[p] = t_div(a.v[p], b.v[p]);
   return a;

@@ -61,8 +61,9 @@ enum fx_op : uint16_t {
   FX_MULM = FX_ADDM + FX_L,           // A[d] = A[d]*M[aux]
   FX_FMA_MC_A = FX_MULM + FX_L,       // A[d] = M[aux]*imm + A[d]
   FX_FMA_AM_C = FX_FMA_MC_A + FX_L,   // A[d] = A[d]*M[aux] + imm
+  FX_FMA_UPC = FX_FMA_AM_C + FX_L,    // A[d] = A[d+1]*imm + A[d]         (d < L-1)
   // level-0 register families
-  FX_SUB_R = FX_FMA_AM_C + FX_L,      // A = A - R[r]
+  FX_SUB_R = FX_FMA_UPC + FX_L,       // A = A - R[r]
   FX_RSUB_R = FX_SUB_R + FX_NR,       // A = R[r] - A
   FX_DIV_R = FX_RSUB_R + FX_NR,       // A = A / R[r]
   FX_RDIV_R = FX_DIV_R + FX_NR,       // A = R[r] / A

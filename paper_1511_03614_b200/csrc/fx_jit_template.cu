@@ -16,7 +16,7 @@
 // hook fiesta_eval_points runs the SAME generated program body as the integration kernels).
 //
 // Marker operand order (fx_jit.cpp parses it):
-//   integrate: nonfinite [h2[0..P) if Vegas] valid acc W[0..P) x[0][0..P) x[1][..) ...
+//   integrate: [h2[0..P) if Vegas] valid acc W[0..P) x[0][0..P) x[1][..) ...
 //   eval:      valid out x[0][0..P) ...
 #define FX_WANT(is_cplx, nx, p) 0  // no interpreter fast path in this translation unit
 #include "fx_device_common.cuh"
@@ -127,10 +127,18 @@ extern "C" __global__ void __launch_bounds__(FX_THREADS, FXJ_BLOCKS)
   fx_block_setup(prm, dim, (uint32_t)sec.sector_id, r, sel_idx, sh_delta, sh_grid, sh_hist);
   const int nslots = 2 * sec.K;
   for (int s = 0; s < nslots; ++s) sh_acc[s * FX_THREADS + threadIdx.x] = 0.0;
+  unsigned *sh_nf = reinterpret_cast<unsigned *>(smem + L.nf);  // non-finite values seen by this thread (the body counts)
+  sh_nf[2 * threadIdx.x] = 0u;
+  if (threadIdx.x == 96) {
+    const uint64_t c0 = (uint64_t)chunk * prm.chunk;
+    const uint64_t c1 = min(c0 + prm.chunk, prm.n_per_shift);
+    uint64_t *rg = fx_block_range(sh_delta);
+    rg[0] = c0;
+    rg[1] = c1;
+    rg[2] = (c1 - c0 + (uint64_t)FX_THREADS * PB - 1) / ((uint64_t)FX_THREADS * PB) * (PB / P);
+  }
   __syncthreads();
 
-  unsigned nonfinite = 0;
-  const uint32_t acc = (uint32_t)__cvta_generic_to_shared(sh_acc + threadIdx.x);
   // The trip count is the same for every thread of the block (points past the end are masked by
   // `valid`), so the block can re-align its warps at every pass: a sector's native code is ~45 KB
   // of straight-line instructions, far beyond the instruction caches, and warps that drift apart
@@ -145,37 +153,42 @@ extern "C" __global__ void __launch_bounds__(FX_THREADS, FXJ_BLOCKS)
   // unchanged (bit-identical to the interpreter's).
   //
   // Pass q covers the points c0 + (q/2) * 512 + 4 tid + 2 (q%2) + {0, 1} (a chunk has at most 2^17 points).
-  const uint64_t c0 = (uint64_t)chunk * prm.chunk;
-  const uint64_t c1 = min(c0 + prm.chunk, prm.n_per_shift);
-  const uint32_t npass = (uint32_t)((c1 - c0 + (uint64_t)FX_THREADS * PB - 1) / ((uint64_t)FX_THREADS * PB)) * (PB / P);
+  // Only q is carried across the program body: the block's range, the thread index and the
+  // accumulator address are read again in every pass (volatile), so that the register allocation
+  // of the body has no loop invariants to hold -- or to spill.
 #pragma unroll 1
-  for (uint32_t q = 0; q < npass; ++q) {
+  for (uint32_t q = 0;; ++q) {
+    const uint64_t *rg = fx_block_range(sh_delta);
+    if (q >= (uint32_t)fx_lds_volatile(rg + 2)) break;
     {
-      const uint64_t base = c0 + (uint64_t)((q / (PB / P)) * (FX_THREADS * PB) + threadIdx.x * PB + (q % (PB / P)) * P);
+      const unsigned tid = fx_tid_volatile();
+      const uint64_t c1 = fx_lds_volatile(rg + 1);
+      const uint64_t base = fx_lds_volatile(rg) + (uint64_t)((q / (PB / P)) * (FX_THREADS * PB) + tid * PB + (q % (PB / P)) * P);
+      const uint32_t acc = (uint32_t)__cvta_generic_to_shared(sh_acc) + tid * 8u;
       __syncthreads();
       double x[NX][P], W[P];
       unsigned valid;
 #if FXJ_MODE == 0
       fxj_make_points<NX, P>(prm, dim, sh_delta, base, c1, x, W, valid);
       asm volatile("FXJIT_BODY " FXJ_FMT ";"
-                   : "+r"(nonfinite)
+                   :
                    : "r"(valid), "r"(acc), "d"(W[0]), "d"(W[1]), FXJ_XS
                    : "memory");
 #else
       double xbar[NX][P];
       uint32_t bins[(NX + 3) / 4][P];
-      fx_make_points<FXJ_RULE, NX, P>(prm, dim, (uint32_t)sec.sector_id, sh_delta, sh_grid, base, c1, x, xbar, W, valid,
+      fx_make_points<FXJ_RULE, NX, P, true>(prm, dim, (uint32_t)sec.sector_id, sh_delta, sh_grid, base, c1, x, xbar, W, valid,
                                       bins);
 #if FXJ_MODE == 2
       double h2[P] = {0.0, 0.0};
       asm volatile("FXJIT_BODY " FXJ_FMT ";"
-                   : "+r"(nonfinite), "+d"(h2[0]), "+d"(h2[1])
+                   : "+d"(h2[0]), "+d"(h2[1])
                    : "r"(valid), "r"(acc), "d"(W[0]), "d"(W[1]), FXJ_XS
                    : "memory");
       fx_hist_points<NX, P>(sh_hist, dim, prm.nbins, valid, bins, h2);
 #else
       asm volatile("FXJIT_BODY " FXJ_FMT ";"
-                   : "+r"(nonfinite)
+                   :
                    : "r"(valid), "r"(acc), "d"(W[0]), "d"(W[1]), FXJ_XS
                    : "memory");
 #endif
@@ -188,6 +201,7 @@ extern "C" __global__ void __launch_bounds__(FX_THREADS, FXJ_BLOCKS)
   }
   __syncthreads();
   const fx_block_id id1 = fx_block_coords(prm);  // again, rather than kept across the loop
+  const unsigned nonfinite = sh_nf[2 * threadIdx.x];
   fx_block_reduce(sh_acc, sh_wsum, 2 * prm.sectors[prm.sel[id1.sel_idx]].K, fx_partial_record(prm, id1.sel_idx, id1.r, id1.chunk));
   fx_block_finish(prm, dim, id1.sel_idx, id1.chunk, nonfinite, sh_hist);
 }

@@ -13,7 +13,7 @@
 //
 // Marker operand order (fx_jit.cpp parses it):
 //   FXJIT_DEFORM  gh[0..NGH) x[0..N)
-//   FXJIT_BODY    integrate: nonfinite [h2 if Vegas] valid acc Wd.re Wd.im z[0].re z[0].im z[1].re ...
+//   FXJIT_BODY    integrate: [h2 if Vegas] valid acc Wd.re Wd.im z[0].re z[0].im z[1].re ...
 //                 eval:      valid out det.re det.im z[0].re z[0].im ...
 // build.py passes the operand lists as macros: FXJ_DFMT / FXJ_FMT ("%0 %1 ..."), FXJ_GH_OUTS
 // ("=d"(gh[0]), ...), FXJ_X_INS ("d"(xv[0]), ...), FXJ_Z_INS ("d"(xv[0]), "d"(zi[0]), ...).
@@ -63,11 +63,12 @@ extern "C" __global__ void __launch_bounds__(FX_THREADS, FXJ_CBLOCKS)
   fx_block_setup(prm, N, (uint32_t)sec.sector_id, r, sel_idx, sh_delta, sh_grid, sh_hist);
   const int nslots = 4 * sec.K;
   for (int s = 0; s < nslots; ++s) sh_acc[s * FX_THREADS + threadIdx.x] = 0.0;
+  unsigned *sh_nf = reinterpret_cast<unsigned *>(smem + L.nf);  // non-finite values seen by this thread (the body counts)
+  sh_nf[2 * threadIdx.x] = 0u;
   __syncthreads();
 
   const uint64_t c0 = (uint64_t)chunk * prm.chunk;
   const uint64_t c1 = min(c0 + prm.chunk, prm.n_per_shift);
-  unsigned nonfinite = 0;
   const uint32_t acc = (uint32_t)__cvta_generic_to_shared(sh_acc + threadIdx.x);
   const bool deform = sec.deform_len != 0;
 #pragma unroll 1
@@ -91,13 +92,13 @@ extern "C" __global__ void __launch_bounds__(FX_THREADS, FXJ_CBLOCKS)
 #if FXJ_MODE == 2
     double h2[P] = {0.0};
     asm volatile("FXJIT_BODY " FXJ_FMT ";"
-                 : "+r"(nonfinite), "+d"(h2[0])
+                 : "+d"(h2[0])
                  : "r"(valid), "r"(acc), "d"(Wd.re), "d"(Wd.im), FXJ_Z_INS
                  : "memory");
     fx_hist_points<N, P>(sh_hist, N, prm.nbins, valid, bins, h2);
 #else
     asm volatile("FXJIT_BODY " FXJ_FMT ";"
-                 : "+r"(nonfinite)
+                 :
                  : "r"(valid), "r"(acc), "d"(Wd.re), "d"(Wd.im), FXJ_Z_INS
                  : "memory");
 #endif
@@ -108,6 +109,7 @@ extern "C" __global__ void __launch_bounds__(FX_THREADS, FXJ_CBLOCKS)
   }
   __syncthreads();
   const fx_block_id id1 = fx_block_coords(prm);  // again, rather than kept across the loop
+  const unsigned nonfinite = sh_nf[2 * threadIdx.x];
   fx_block_reduce(sh_acc, sh_wsum, 4 * prm.sectors[prm.sel[id1.sel_idx]].K, fx_partial_record(prm, id1.sel_idx, id1.r, id1.chunk));
   fx_block_finish(prm, N, id1.sel_idx, id1.chunk, nonfinite, sh_hist);
 }

@@ -10,7 +10,7 @@
 #define FX_THREADS 128   // threads per block of the evaluation kernels
 #define FX_P_REAL 4      // points per thread, real programs
 #define FX_P_CPLX 1      // points per thread, complex programs
-#define FX_TF_BYTES (80u + FX_NXMAX * 8u)  // shared memory: fx_transform, then the lattice steps G_k
+#define FX_TF_BYTES (80u + FX_NXMAX * 8u + 32u)  // shared memory: fx_transform, the lattice steps G_k, the block's point range
 #define FX_ACC_SLOTS 32  // per-(sector,shift,chunk) partial record: [K<=8][C<=2][S1,S2]
 
 struct fx_sector_dev {       // one compiled sector in the device arena
@@ -93,12 +93,13 @@ size_t fx_integrate_smem_bytes(const fx_integrate_params &p);
 #define FXJ_ACC_SLOTS 32
 #define FXJ_P 2  // points per thread and pass of the native program body (two passes per batch of FX_P_REAL)
 struct fxj_smem_layout {
-  uint32_t acc, delta, tf, grid, hist, wsum, total;
+  uint32_t acc, nf, delta, tf, grid, hist, wsum, total;
 };
 static inline __host__ __device__ fxj_smem_layout fxj_layout(int dim, int nbins, bool vegas, int acc_slots = 16) {
   fxj_smem_layout L;
   L.acc = 0;
-  L.delta = (uint32_t)acc_slots * FX_THREADS * 8u;
+  L.nf = (uint32_t)acc_slots * FX_THREADS * 8u;  // per-thread count of non-finite values, right behind the accumulators
+  L.delta = L.nf + FX_THREADS * 8u;
   L.tf = L.delta + FX_NXMAX * 8u;
   L.grid = L.tf + FX_TF_BYTES;
   L.hist = L.grid + (vegas ? (uint32_t)dim * (nbins + 1) * 8u : 0u);

@@ -191,7 +191,7 @@ class Gen:
         isx = r is not None and r < NXMAX
         if fam in ("MULC_R", "MUL_R", "FMA_AR_C", "FMA_RC_A", "FMA_UP") and isx:
             return 0
-        if fam in ("LDC", "ADDC", "MULC", "ADD_UP", "MUL_UP", "ST_S", "NEG", "SQR", "RSUBC"):
+        if fam in ("LDC", "ADDC", "MULC", "ADD_UP", "MUL_UP", "FMA_UPC", "ST_S", "NEG", "SQR", "RSUBC"):
             return 1
         if "DIV" in fam or fam == "SQRT":
             return 9
@@ -269,6 +269,7 @@ class Gen:
         l_family("MULM", lambda a, d, p: self.mul(a, self.ld_mem(p)), self.mem_addr)
         l_family("FMA_MC_A", lambda a, d, p: self.fma_rc(a, self.ld_mem(p)), self.mem_addr)
         l_family("FMA_AM_C", lambda a, d, p: self.fma_c(a, self.ld_mem(p)), self.mem_addr)
+        l_family("FMA_UPC", lambda a, d, p: self.fma_rc(a, AL[d + 1][p]), dmax=NL - 1)
 
         r0_family("SUB_R", lambda a, r, p: self.comp2("sub.rn.f64", a, a, r))
         r0_family("RSUB_R", lambda a, r, p: self.comp2("sub.rn.f64", a, r, a))
