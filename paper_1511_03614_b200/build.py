@@ -22,6 +22,7 @@ ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 NVFLAGS = ["-O3", "-std=c++17", "-lineinfo", "-fmad=false", "-Xcompiler", "-fPIC", "-Xptxas", "-v"] + ARCH
 CPLX_DIMS = range(1, 9)
 JIT_NX = (4, 8, 12)
+P_VEGAS = int(os.environ.get("FXJ_P_VEGAS", "1"))   # points per pass of the native Vegas kernels (fx_kernels.h)
 # resident blocks per SM the native complex kernels are held to (register budget 65536 / (128 * blocks))
 CPLX_BLOCKS = {1: 6, 2: 6, 3: 5, 4: 4, 5: 3, 6: 3, 7: 2, 8: 2}
 
@@ -81,8 +82,12 @@ def build(force=False, verbose=False):
                         "FXJ_CBLOCKS": CPLX_BLOCKS[n]}
                 src = tpl_srcs[1]
             else:
-                nbody = (2 if mode == 3 else (6 if mode == 2 else 4)) + 2 * n
-                defs = {"FXJ_NX": n, "FXJ_FMT": fmt(nbody)}
+                P = P_VEGAS if mode == 2 else 2
+                nbody = (2 if mode == 3 else (2 * P + 2 if mode == 2 else P + 2)) + P * n
+                defs = {"FXJ_NX": n, "FXJ_FMT": fmt(nbody), "FXJ_P_VEGAS": P_VEGAS,
+                        "FXJ_XS": ", ".join('"d"(x[%d][%d])' % (k, p) for k in range(n) for p in range(P)),
+                        "FXJ_WS": ", ".join('"d"(W[%d])' % p for p in range(P)),
+                        "FXJ_H2S": ", ".join('"+d"(h2[%d])' % p for p in range(P))}
                 src = tpl_srcs[0]
             defs["FXJ_MODE"] = mode
             hdr = out[:-4] + "_defs.h"   # operand lists contain commas: a header, not -D
@@ -121,7 +126,8 @@ def build(force=False, verbose=False):
     for name in ("fiesta_abi", "fx_compiler", "fx_jit"):
         o = os.path.join(OBJ, name + ".o")
         s = os.path.join(CSRC, name + ".cpp")
-        jobs.append((o, ["g++", "-O2", "-std=c++17", "-fPIC", "-pthread", "-I/usr/local/cuda/include", "-c", s, "-o", o],
+        jobs.append((o, ["g++", "-O2", "-std=c++17", "-fPIC", "-pthread", "-DFXJ_P_VEGAS=%d" % P_VEGAS,
+                         "-I/usr/local/cuda/include", "-c", s, "-o", o],
                      [s] + hdrs + ([tpl_inc] if name == "fx_jit" else [])))
     todo = [(o, c) for (o, c, srcs) in jobs if force or _stale(o, srcs)]
     if verbose and todo:

@@ -278,7 +278,7 @@ bool assemble_cached(const fx::CompiledSector &cs, int mode, std::string &cubin,
 
 size_t native_smem_max(const fiesta_program *pg, const fx::CompiledSector &cs, int mode) {
   const bool vegas = mode == fx::JIT_VEGAS;
-  const size_t want = fxj_layout(cs.dim, FIESTA_MAX_BINS, vegas, cs.is_complex ? FXJ_ACC_SLOTS : 16).total;
+  const size_t want = fxj_layout(cs.dim, FIESTA_MAX_BINS, vegas, fxj_acc_slots(vegas, cs.is_complex, cs.K)).total;
   return mode == fx::JIT_EVAL ? 0 : std::min(want, pg->smem_optin);
 }
 

@@ -388,6 +388,7 @@ struct Lowering {
   const RawDag &raw;
   const std::set<int> &fbound;
   int dim;
+  bool cplx = false;
   std::vector<LNode> nodes;
   std::map<int, int> memo;   // raw id -> lowered id (as a root)
   std::map<int, int> memo2;  // raw id -> lowered id (as an operand)
@@ -422,6 +423,74 @@ struct Lowering {
     x.terms = p;
     nodes.push_back(x);
     return (int)nodes.size() - 1;
+  }
+  // node id = exp(q*log a), i.e. a real power a^q (R_POWR below): base a and exponent q
+  bool as_real_power(int id, int &base, double &q) const {
+    if (id < dim || nodes[id].k != L_EXP) return false;
+    const LNode &arg = nodes[nodes[id].a];
+    if (arg.k != L_POLY || arg.terms.size() != 1 || arg.terms[0].f.size() != 1 || arg.terms[0].f[0].second != 1) return false;
+    const int ll = arg.terms[0].f[0].first;
+    if (ll < dim || nodes[ll].k != L_LOG) return false;
+    base = nodes[ll].a;
+    q = arg.terms[0].c;
+    return true;
+  }
+  // a variable, or a product of variables with coefficient 1: positive on the integration domain (0,1)^n
+  bool variable_monomial(int id, Term &m) const {
+    if (id < dim) {
+      m = Term{1.0, {{id, 1}}};
+      return true;
+    }
+    const LNode &n = nodes[id];
+    if (n.k != L_POLY || n.terms.size() != 1 || n.terms[0].c != 1.0) return false;
+    for (auto &fe : n.terms[0].f)
+      if (fe.first >= dim) return false;
+    m = n.terms[0];
+    return true;
+  }
+  // Real arithmetic only: x_i^q * x_j^q -> (x_i x_j)^q for variables (and products of variables), one
+  // log and one exp instead of one pair per factor.  The variables are positive on the integration
+  // domain, the open unit cube (R2: u in (0,1)), where the two forms are the same function;
+  // a caller of fiesta_eval_points with x <= 0 gets NaN from either unless an even number of the
+  // merged variables is negative.  Not done in complex mode (branch cuts).
+  void merge_real_powers(Term &t) {
+    if (cplx) return;
+    for (;;) {
+      int i0 = -1, i1 = -1;
+      for (size_t i = 0; i < t.f.size() && i1 < 0; ++i) {
+        int bi;
+        double qi;
+        Term mi;
+        if (t.f[i].second != 1 || !as_real_power(t.f[i].first, bi, qi) || !variable_monomial(bi, mi)) continue;
+        for (size_t j = i + 1; j < t.f.size(); ++j) {
+          int bj;
+          double qj;
+          Term mj;
+          if (t.f[j].second != 1 || !as_real_power(t.f[j].first, bj, qj) || qj != qi || !variable_monomial(bj, mj)) continue;
+          i0 = (int)i;
+          i1 = (int)j;
+          break;
+        }
+      }
+      if (i1 < 0) return;
+      int b0, b1;
+      double q, q1;
+      Term m0, m1;
+      as_real_power(t.f[i0].first, b0, q);
+      as_real_power(t.f[i1].first, b1, q1);
+      variable_monomial(b0, m0);
+      variable_monomial(b1, m1);
+      const int prod = from_poly(Poly{mul_terms(m0, m1)});
+      const int ll = make(L_LOG, prod, -1, 0, 0);
+      const int arg = from_poly(Poly{Term{q, {{ll, 1}}}});
+      const int e = make(L_EXP, arg, -1, 0, 0);
+      t.f.erase(t.f.begin() + i1);
+      t.f.erase(t.f.begin() + i0);
+      Term one{1.0, {{e, 1}}};
+      const double c = t.c;
+      t = mul_terms(t, one);
+      t.c = c;
+    }
   }
   Poly atom_poly(int lid) {
     if (nodes[lid].k == L_CONST) {
@@ -468,7 +537,10 @@ struct Lowering {
         const Poly &mono = p.size() == 1 ? p : q;
         const Poly &other = p.size() == 1 ? q : p;
         Poly out;
-        for (auto &t : other) out.push_back(mul_terms(mono[0], t));
+        for (auto &t : other) {
+          out.push_back(mul_terms(mono[0], t));
+          merge_real_powers(out.back());
+        }
         normalize(out);
         return out;
       }
@@ -1158,6 +1230,7 @@ CompiledSector compile_sector(const char *const *texts, int K, int dim, bool is_
   if (deform_f_index > 0 && !(lambda >= 0.0)) fail(FIESTA_E_ARG, "lambda must be >= 0 (PAPER.md:474: Im F(z) < 0 needs a positive deformation)");
 
   Lowering low(raw, fbound, dim);
+  low.cplx = cs.is_complex;
   std::vector<int> lroots(K);
   for (int k = 0; k < K; ++k) lroots[k] = low.lower(roots[k]);
   {

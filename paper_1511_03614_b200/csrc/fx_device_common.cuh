@@ -102,15 +102,15 @@ static __device__ __noinline__ fx_coordP<P> fx_lattice_coord(fx_tP<P> t, const f
   return fx_lattice_coord_body<P>(t, tf);
 }
 
-__device__ __forceinline__ fx_tpair fx_philox_pair_body(uint64_t seed, uint32_t sector_id, uint32_t tag, uint32_t it,
+__device__ __forceinline__ fx_tpair fx_philox_pair_body(const uint32_t *rk, uint32_t sector_id, uint32_t tag, uint32_t it,
                                                         uint64_t j, uint32_t kb) {
   fx_tpair r;
-  philox_t_pair(seed, sector_id, tag, it, j, kb, r.e, r.o);
+  philox_t_pair_rk(rk, sector_id, tag, it, j, kb, r.e, r.o);
   return r;
 }
-static __device__ __noinline__ fx_tpair fx_philox_pair(uint64_t seed, uint32_t sector_id, uint32_t tag, uint32_t it, uint64_t j,
-                                                uint32_t kb) {
-  return fx_philox_pair_body(seed, sector_id, tag, it, j, kb);
+static __device__ __noinline__ fx_tpair fx_philox_pair(const uint32_t *rk, uint32_t sector_id, uint32_t tag, uint32_t it,
+                                                       uint64_t j, uint32_t kb) {
+  return fx_philox_pair_body(rk, sector_id, tag, it, j, kb);
 }
 
 struct fx_vcoord {
@@ -172,8 +172,8 @@ __device__ __forceinline__ void fx_make_points(const fx_integrate_params &prm, i
       FX_PLOOP {
         fx_tpair tp{0ull, 0ull};
         if (2 * kb < dim)
-          tp = INL ? fx_philox_pair_body(prm.seed, sector_id, FX_TAG_MC, (uint32_t)prm.iteration, j0 + p, kb)
-                   : fx_philox_pair(prm.seed, sector_id, FX_TAG_MC, (uint32_t)prm.iteration, j0 + p, kb);
+          tp = INL ? fx_philox_pair_body(prm.philox_rk, sector_id, FX_TAG_MC, (uint32_t)prm.iteration, j0 + p, kb)
+                   : fx_philox_pair(prm.philox_rk, sector_id, FX_TAG_MC, (uint32_t)prm.iteration, j0 + p, kb);
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
           const int k = 2 * kb + h;
@@ -209,7 +209,7 @@ __device__ __forceinline__ void fx_block_setup(const fx_integrate_params &prm, i
   if (threadIdx.x < (FX_NXMAX + 1) / 2) {
     uint64_t te = 0, to = 0;
     if (prm.rule == FIESTA_RULE_LATTICE)
-      philox_t_pair(prm.seed, sector_id, FX_TAG_SHIFT, (uint32_t)r, 0ull, threadIdx.x, te, to);
+      philox_t_pair_rk(prm.philox_rk, sector_id, FX_TAG_SHIFT, (uint32_t)r, 0ull, threadIdx.x, te, to);
     sh_delta[2 * threadIdx.x] = te;
     sh_delta[2 * threadIdx.x + 1] = to;
   }
@@ -232,52 +232,41 @@ __device__ __forceinline__ void fx_block_setup(const fx_integrate_params &prm, i
   }
 }
 
-// Vegas histogram (R8): h[k][bin] += v for one point per lane, into the
-// WARP's own histogram in shared memory.  Warp-aggregated: the lanes whose points fall into the
-// same bin of dimension k are found with match.any; each group is a linked list in lane order
-// (next = the next higher lane of the group), and its values are added by pointer jumping -- every
-// lane adds the value of its successor and then points to its successor's successor, so after
-// ceil(log2(group size)) steps the group's first lane holds the group's sum, in a summation tree
-// fixed by the lanes' positions alone; that lane then does one plain read-modify-write.  No atomics,
-// every addition in a fixed order: the histogram -- like the sums -- is bit-reproducible.
-__device__ __forceinline__ unsigned fx_hist_peers(unsigned bin, bool valid) {
-  const unsigned lane = threadIdx.x & 31u;
-  return __match_any_sync(0xffffffffu, valid ? bin : (0x100u | lane));  // a point past the end matches nobody
-}
-__device__ __forceinline__ void fx_hist_add(double *warp_hist_k /* this warp's h[k][0..nbins) */, unsigned bin,
-                                            unsigned peers, double v, bool valid) {
-  const unsigned full = 0xffffffffu;
-  const unsigned lane = threadIdx.x & 31u;
-  const unsigned below = (1u << lane) - 1u;
-  const unsigned higher = peers & ~(below | (1u << lane));
-  int nxt = higher ? (__ffs(higher) - 1) : -1;
-  while (__any_sync(full, nxt >= 0)) {
-    const int src = nxt >= 0 ? nxt : (int)lane;
-    const double t = __shfl_sync(full, v, src);
-    const int n2 = __shfl_sync(full, nxt, src);
-    if (nxt >= 0) {
-      v += t;
-      nxt = n2;
-    }
-  }
-  if (valid && (peers & below) == 0u) warp_hist_k[bin] += v;
-}
-
-// all dimensions of the P points of a thread, point by point (the order both tiers use)
+// Vegas histogram (R8): h[k][bin_k] += v for one point per lane and every
+// dimension k, into the WARP's own histogram in shared memory.  Warp-aggregated: the lanes whose
+// points fall into the same bin of dimension k are found with match.any, and a lane's rank in its
+// group is the number of group members on lower lanes.  The warp then takes turns by rank: in turn s
+// the lanes of rank s do a plain read-modify-write of their cell, for all dimensions at once (cells
+// of different dimensions are different words), with a warp barrier between turns.  Two lanes never
+// touch one cell in the same turn, a cell receives its contributions in lane order, and there is no
+// atomic anywhere: the histogram -- like the sums -- is bit-reproducible.  The number of turns is the
+// largest group (3-4 for 32 lanes in 50 bins).
 template <int NX, int P>
 __device__ __forceinline__ void fx_hist_points(double *sh_hist, int dim, int nbins, unsigned valid,
                                                const uint32_t (&bins)[(NX + 3) / 4][P], const double (&h2)[P]) {
+  const unsigned full = 0xffffffffu;
+  const unsigned lane = threadIdx.x & 31u;
+  const unsigned below = (1u << lane) - 1u;
   double *wh = sh_hist + (size_t)(threadIdx.x >> 5) * dim * nbins;
-  FX_PLOOP {
+  FX_PLOOP {  // point by point: the order both tiers use
     const bool ok = (valid >> p) & 1u;
-    unsigned peers[NX];  // all matches first: their latencies overlap
+    unsigned rank[NX];  // all matches first: their latencies overlap
+    unsigned turns = 0;
 #pragma unroll
     for (int k = 0; k < NX; ++k)
-      if (k < dim) peers[k] = fx_hist_peers((bins[k / 4][p] >> (8 * (k % 4))) & 0xffu, ok);
+      if (k < dim) {
+        const unsigned bin = (bins[k / 4][p] >> (8 * (k % 4))) & 0xffu;
+        const unsigned peers = __match_any_sync(full, ok ? bin : (0x100u | lane));  // a point past the end matches nobody
+        rank[k] = ok ? (unsigned)__popc(peers & below) : 0xffffu;
+        turns = max(turns, ok ? rank[k] + 1u : 0u);
+      }
+    turns = __reduce_max_sync(full, turns);
+    for (unsigned s = 0; s < turns; ++s) {
 #pragma unroll
-    for (int k = 0; k < NX; ++k)
-      if (k < dim) fx_hist_add(wh + k * nbins, (bins[k / 4][p] >> (8 * (k % 4))) & 0xffu, peers[k], h2[p], ok);
-    __syncwarp();  // the next point's read-modify-writes (other lanes, same cells) come after these
+      for (int k = 0; k < NX; ++k)
+        if (k < dim && rank[k] == s) wh[k * nbins + ((bins[k / 4][p] >> (8 * (k % 4))) & 0xffu)] += h2[p];
+      __syncwarp();
+    }
   }
 }
 

@@ -82,19 +82,10 @@ __device__ __forceinline__ void fxj_make_points(const fx_integrate_params &prm, 
   FX_PLOOP { W[p] = korobov_weight(*tf, W[p]); }
 }
 
-#define FXJ_X2(k) "d"(x[k][0]), "d"(x[k][1])
-#if FXJ_NX == 4
-#define FXJ_XS FXJ_X2(0), FXJ_X2(1), FXJ_X2(2), FXJ_X2(3)
-#elif FXJ_NX == 8
-#define FXJ_XS FXJ_X2(0), FXJ_X2(1), FXJ_X2(2), FXJ_X2(3), FXJ_X2(4), FXJ_X2(5), FXJ_X2(6), FXJ_X2(7)
-#else
-#define FXJ_XS                                                                                             \
-  FXJ_X2(0), FXJ_X2(1), FXJ_X2(2), FXJ_X2(3), FXJ_X2(4), FXJ_X2(5), FXJ_X2(6), FXJ_X2(7), FXJ_X2(8), FXJ_X2(9), \
-      FXJ_X2(10), FXJ_X2(11)
-#endif
-// FXJ_FMT ("%0 %1 ... %(n-1)": the marker line lists every operand once, in order) comes from build.py
-#ifndef FXJ_FMT
-#error "build.py passes -DFXJ_FMT"
+// FXJ_FMT ("%0 %1 ... %(n-1)": the marker line lists every operand once, in order) and the operand lists
+// FXJ_XS ("d"(x[0][0]), ...), FXJ_WS ("d"(W[0]), ...), FXJ_H2S ("+d"(h2[0]), ...) come from build.py
+#if !defined(FXJ_FMT) || !defined(FXJ_XS) || !defined(FXJ_WS) || !defined(FXJ_H2S)
+#error "build.py passes FXJ_FMT, FXJ_XS, FXJ_WS, FXJ_H2S"
 #endif
 
 #if FXJ_MODE != 3
@@ -103,21 +94,21 @@ constexpr int FXJ_RULE = FXJ_MODE;
 // resident blocks per SM the register allocation is held to: the most for which the assembler reports
 // no spill on the configurations' programs (lattice: 6 x 80 registers at NX <= 8; plain MC carries
 // the Philox state on top: 5 x 96; Vegas also the bins and h2: 4 x 128)
-constexpr int FXJ_BLOCKS = FXJ_MODE == 2 ? 4 : FXJ_MODE == 1 ? (FXJ_NX <= 8 ? 5 : 4) : (FXJ_NX <= 8 ? 6 : 4);
+constexpr int FXJ_BLOCKS = FXJ_MODE == 2 ? (FXJ_P_VEGAS == 1 ? 6 : 4) : FXJ_MODE == 1 ? (FXJ_NX <= 8 ? 5 : 4) : (FXJ_NX <= 8 ? 6 : 4);
 
 extern "C" __global__ void __launch_bounds__(FX_THREADS, FXJ_BLOCKS)
     fxj_integrate(const __grid_constant__ fx_integrate_params prm) {
   constexpr int PB = FX_P_REAL;  // points per thread and batch: the interpreter's
-  constexpr int P = FXJ_P;       // points per pass of the program body
+  constexpr int P = FXJ_P_OF(FXJ_MODE);  // points per pass of the program body
   constexpr int NX = FXJ_NX;
   constexpr bool vegas = FXJ_RULE == FIESTA_RULE_VEGAS;
-  static_assert(P == 2 && PB % P == 0, "the marker lists 2 points per variable");
+  static_assert(PB % P == 0, "a batch is a whole number of passes");
   extern __shared__ __align__(16) unsigned char smem[];
   const fx_block_id id0 = fx_block_coords(prm);
   const int chunk = id0.chunk, r = id0.r, sel_idx = id0.sel_idx;
   const fx_sector_dev sec = prm.sectors[prm.sel[sel_idx]];
   const int dim = prm.dim;
-  const fxj_smem_layout L = fxj_layout(dim, prm.nbins, vegas);
+  const fxj_smem_layout L = fxj_layout(dim, prm.nbins, vegas, fxj_acc_slots(vegas, false, sec.K));
   double *sh_acc = reinterpret_cast<double *>(smem + L.acc);
   uint64_t *sh_delta = reinterpret_cast<uint64_t *>(smem + L.delta);
   double *sh_grid = reinterpret_cast<double *>(smem + L.grid);
@@ -152,7 +143,7 @@ extern "C" __global__ void __launch_bounds__(FX_THREADS, FXJ_BLOCKS)
   // accumulated (and, for Vegas, histogrammed) in point order either way, so the sums are
   // unchanged (bit-identical to the interpreter's).
   //
-  // Pass q covers the points c0 + (q/2) * 512 + 4 tid + 2 (q%2) + {0, 1} (a chunk has at most 2^17 points).
+  // Pass q covers the points c0 + (q / (PB/P)) * 512 + PB tid + P (q % (PB/P)) + {0..P-1} (a chunk has at most 2^17 points).
   // Only q is carried across the program body: the block's range, the thread index and the
   // accumulator address are read again in every pass (volatile), so that the register allocation
   // of the body has no loop invariants to hold -- or to spill.
@@ -172,7 +163,7 @@ extern "C" __global__ void __launch_bounds__(FX_THREADS, FXJ_BLOCKS)
       fxj_make_points<NX, P>(prm, dim, sh_delta, base, c1, x, W, valid);
       asm volatile("FXJIT_BODY " FXJ_FMT ";"
                    :
-                   : "r"(valid), "r"(acc), "d"(W[0]), "d"(W[1]), FXJ_XS
+                   : "r"(valid), "r"(acc), FXJ_WS, FXJ_XS
                    : "memory");
 #else
       double xbar[NX][P];
@@ -180,16 +171,17 @@ extern "C" __global__ void __launch_bounds__(FX_THREADS, FXJ_BLOCKS)
       fx_make_points<FXJ_RULE, NX, P, true>(prm, dim, (uint32_t)sec.sector_id, sh_delta, sh_grid, base, c1, x, xbar, W, valid,
                                       bins);
 #if FXJ_MODE == 2
-      double h2[P] = {0.0, 0.0};
+      double h2[P];
+      FX_PLOOP { h2[p] = 0.0; }
       asm volatile("FXJIT_BODY " FXJ_FMT ";"
-                   : "+d"(h2[0]), "+d"(h2[1])
-                   : "r"(valid), "r"(acc), "d"(W[0]), "d"(W[1]), FXJ_XS
+                   : FXJ_H2S
+                   : "r"(valid), "r"(acc), FXJ_WS, FXJ_XS
                    : "memory");
       fx_hist_points<NX, P>(sh_hist, dim, prm.nbins, valid, bins, h2);
 #else
       asm volatile("FXJIT_BODY " FXJ_FMT ";"
                    :
-                   : "r"(valid), "r"(acc), "d"(W[0]), "d"(W[1]), FXJ_XS
+                   : "r"(valid), "r"(acc), FXJ_WS, FXJ_XS
                    : "memory");
 #endif
 #endif
@@ -209,7 +201,7 @@ extern "C" __global__ void __launch_bounds__(FX_THREADS, FXJ_BLOCKS)
 #else  // FXJ_MODE == 3: the program body on the caller's points (fiesta_eval_points, native tier)
 
 extern "C" __global__ void __launch_bounds__(FX_THREADS) fxj_eval(const __grid_constant__ fx_eval_params prm) {
-  constexpr int P = FXJ_P;
+  constexpr int P = FXJ_P_OF(FXJ_MODE);
   constexpr int NX = FXJ_NX;
   const fx_sector_dev sec = prm.sectors[prm.sector];
   const uint64_t first = ((uint64_t)blockIdx.x * FX_THREADS + threadIdx.x) * P;

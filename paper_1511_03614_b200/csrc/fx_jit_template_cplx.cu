@@ -53,7 +53,7 @@ extern "C" __global__ void __launch_bounds__(FX_THREADS, FXJ_CBLOCKS)
   const fx_block_id id0 = fx_block_coords(prm);
   const int chunk = id0.chunk, r = id0.r, sel_idx = id0.sel_idx;
   const fx_sector_dev sec = prm.sectors[prm.sel[sel_idx]];
-  const fxj_smem_layout L = fxj_layout(N, prm.nbins, vegas, FXJ_ACC_SLOTS);
+  const fxj_smem_layout L = fxj_layout(N, prm.nbins, vegas, fxj_acc_slots(vegas, true, sec.K));
   double *sh_acc = reinterpret_cast<double *>(smem + L.acc);
   uint64_t *sh_delta = reinterpret_cast<uint64_t *>(smem + L.delta);
   double *sh_grid = reinterpret_cast<double *>(smem + L.grid);

@@ -49,6 +49,7 @@ struct fx_integrate_params {
   uint64_t genvec[FX_NXMAX];
   fx_transform_host tf;
   uint64_t seed;
+  uint32_t philox_rk[20];    // Philox round keys of `seed`: (lo32 + r W0, hi32 + r W1), r = 0..9 (R3)
   int32_t nbins;
   const double *grid;        // Vegas: [nsel][dim][nbins+1]
   double *hist_part;         // Vegas: per-block histograms of this batch [batch sector][nchunks][dim][nbins]
@@ -92,10 +93,20 @@ size_t fx_integrate_smem_bytes(const fx_integrate_params &p);
 // the block reduction's per-warp sums.  No program and no spill slots: both are registers.
 #define FXJ_ACC_SLOTS 32
 #define FXJ_P 2  // points per thread and pass of the native program body (two passes per batch of FX_P_REAL)
+#ifndef FXJ_P_VEGAS
+#define FXJ_P_VEGAS 1  // ... of the Vegas kernels: 12 x[] + bins + Philox state per point; one point keeps 6 blocks resident
+#endif
+#define FXJ_P_OF(mode) ((mode) == 2 ? FXJ_P_VEGAS : FXJ_P)
 struct fxj_smem_layout {
   uint32_t acc, nf, delta, tf, grid, hist, wsum, total;
 };
-static inline __host__ __device__ fxj_smem_layout fxj_layout(int dim, int nbins, bool vegas, int acc_slots = 16) {
+// accumulator slots of a native kernel: a fixed 16 (real) / 32 (complex) for the lattice and MC kernels (every
+// shared-memory offset is then a compile-time constant), exactly 2K / 4K for the Vegas kernels, whose
+// per-warp histograms want the room
+static inline __host__ __device__ int fxj_acc_slots(bool vegas, bool cplx, int K) {
+  return vegas ? (cplx ? 4 : 2) * K : (cplx ? FXJ_ACC_SLOTS : 16);
+}
+static inline __host__ __device__ fxj_smem_layout fxj_layout(int dim, int nbins, bool vegas, int acc_slots) {
   fxj_smem_layout L;
   L.acc = 0;
   L.nf = (uint32_t)acc_slots * FX_THREADS * 8u;  // per-thread count of non-finite values, right behind the accumulators

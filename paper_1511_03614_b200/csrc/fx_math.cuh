@@ -121,6 +121,30 @@ __device__ __forceinline__ philox_out philox4x32_10(uint32_t c0, uint32_t c1, ui
   return o;
 }
 
+// The same ten rounds with the round keys (k0 + r W0, k1 + r W1), r = 0..9, given: rk[2r], rk[2r+1].
+// The evaluation kernels take them from their launch parameters (constant bank): the key schedule is
+// the same for every call of a launch and costs nothing per point that way.
+__device__ __forceinline__ philox_out philox4x32_10_rk(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                                       const uint32_t *rk) {
+  const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    uint32_t hi0 = __umulhi(M0, c0), lo0 = M0 * c0;
+    uint32_t hi1 = __umulhi(M1, c2), lo1 = M1 * c2;
+    uint32_t n0 = hi1 ^ c1 ^ rk[2 * r], n2 = hi0 ^ c3 ^ rk[2 * r + 1];
+    c0 = n0;
+    c1 = lo1;
+    c2 = n2;
+    c3 = lo0;
+  }
+  philox_out o;
+  o.v[0] = c0;
+  o.v[1] = c1;
+  o.v[2] = c2;
+  o.v[3] = c3;
+  return o;
+}
+
 #define FX_TAG_SHIFT 0u
 #define FX_TAG_MC 1u
 
@@ -129,6 +153,13 @@ __device__ __forceinline__ void philox_t_pair(uint64_t seed, uint32_t sector_id,
                                               uint32_t kb, uint64_t &t_even, uint64_t &t_odd) {
   philox_out o = philox4x32_10((uint32_t)j, (uint32_t)(j >> 32), sector_id, (tag << 28) | (kb << 20) | it,
                                (uint32_t)seed, (uint32_t)(seed >> 32));
+  t_even = ((uint64_t)o.v[0] << 32) | o.v[1];
+  t_odd = ((uint64_t)o.v[2] << 32) | o.v[3];
+}
+
+__device__ __forceinline__ void philox_t_pair_rk(const uint32_t *rk, uint32_t sector_id, uint32_t tag, uint32_t it,
+                                                 uint64_t j, uint32_t kb, uint64_t &t_even, uint64_t &t_odd) {
+  philox_out o = philox4x32_10_rk((uint32_t)j, (uint32_t)(j >> 32), sector_id, (tag << 28) | (kb << 20) | it, rk);
   t_even = ((uint64_t)o.v[0] << 32) | o.v[1];
   t_odd = ((uint64_t)o.v[2] << 32) | o.v[3];
 }

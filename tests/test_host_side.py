@@ -180,14 +180,15 @@ def test_native_lowering_keeps_every_operation(lib, name):
         n_call = ptx.count("call.uni")
         assert min(n_fma, n_mul, n_add) >= 0 and (n_fma + n_mul + n_add + n_div + n_call) % 2 == 0
         assert n_fma > 0 and n_call % 2 == 0
-        # the eval kernel and the Vegas kernel are assembled from the same arithmetic
-        for mode in (lib.RULE_VEGAS, lib.MODE_EVAL):
+        # the eval kernel and the Vegas kernel are assembled from the same arithmetic (the Vegas kernel walks
+        # one point per pass, the others two)
+        for mode, pts in ((lib.RULE_VEGAS, 1), (lib.MODE_EVAL, 2)):
             ptx2, _, _ = lib.native_assemble(s, wl.dim, mode)
-            sink_fma = {lib.RULE_VEGAS: 2 * n_out, lib.MODE_EVAL: 0}[mode]      # sum g^2 (+ h2 for Vegas)
-            sink_mul = {lib.RULE_VEGAS: n_out, lib.MODE_EVAL: 0}[mode]
-            assert _count(ptx2, "fma.rn.f64") - sink_fma == n_fma
-            assert _count(ptx2, "mul.rn.f64") - sink_mul == n_mul
-            assert ptx2.count("call.uni") == n_call
+            sink_fma = {lib.RULE_VEGAS: 2 * K * pts, lib.MODE_EVAL: 0}[mode]      # sum g^2 (+ h2 for Vegas)
+            sink_mul = {lib.RULE_VEGAS: K * pts, lib.MODE_EVAL: 0}[mode]
+            assert (_count(ptx2, "fma.rn.f64") - sink_fma) * 2 == n_fma * pts
+            assert (_count(ptx2, "mul.rn.f64") - sink_mul) * 2 == n_mul * pts
+            assert ptx2.count("call.uni") * 2 == n_call * pts
 
 
 def test_native_lowering_of_complex_sectors(lib):
