@@ -203,9 +203,10 @@ def path_overhead_flops(wl):
       A2 lattice, r = 3, per coordinate: v (1), Horner of phi_3 (3 fma), v^4 (2), p (1), 1-p (1), u(1-u) (fma),
          W *= . (1) = 14;  per point: W = cw^n S^3 (3)
       A3 Vegas, per coordinate: fraction (3), width (1), x (fma), weight (2) = 8
-      A4 deformation, dimension n: per k: ls (2), Im z (1), sqrt (15), diagonal (mul, mul, fma = 4); per pair
-         l < k: 2;  elimination of I - iS: per column the pivot (cmul 6, reciprocal 3 + 15 + 2), per row below a
-         complex multiply (6) and one complex fma (8) per entry of the lower triangle
+      A4 deformation, dimension n: per k: ls (2), Im z (1), sqrt (8), diagonal (mul, mul, fma = 4); per pair
+         l < k: 2;  elimination of I - iS: per column the pivot (cmul 6, reciprocal 3 + 10 + 2), per row below a
+         complex multiply (6) and one complex fma (8) per entry of the lower triangle.  (sqrt and the
+         reciprocal at what the routines execute, so that the count stays below ncu's executed flops.)
       A6 per order: real g = W o (1), S1 (1), S2 (fma) = 4 [+ h2 (fma) for Vegas];
          complex g = (W det) o (6), S1, S2 of Re and Im (6) = 12, and W det (2) per point
     Point generation itself (A1) is integer work and is not counted."""
@@ -217,9 +218,9 @@ def path_overhead_flops(wl):
     elif wl.rule == 2:
         f += 8 * n
     if cplx and wl.sectors[0].deform_f_index:
-        f += n * 22 + n * (n - 1)
+        f += n * 15 + n * (n - 1)
         for c in range(n):
-            f += 6 + (20 if c + 1 < n else 0)
+            f += 6 + (15 if c + 1 < n else 0)
             for r in range(c + 1, n):
                 f += 6 + 8 * (r - c)
     f += (12 * K + 2) if cplx else 4 * K

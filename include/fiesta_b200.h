@@ -78,7 +78,7 @@ typedef struct {
   int32_t n_fp64_ops;        /* of which FP64 arithmetic (fma/mul/add/div/log/exp ...)             */
   int32_t n_fma;             /* fused multiply-adds                                                */
   int32_t n_log, n_exp, n_div;
-  int32_t n_reg_temps;       /* register temporaries used (of 8)                                   */
+  int32_t n_reg_temps;       /* register temporaries S[] used (the ISA has FX_NS = 1)              */
   int32_t n_mem_slots;       /* shared-memory spill slots per point (compiler-directed; 0 is best) */
   int32_t n_deform_ops;      /* instructions of the gradient/Hessian program (0 if none)           */
   double flops;              /* FP64 flops per point counted as fma=2, mul/add=1, div=~15, log/exp~40 (nominal) */

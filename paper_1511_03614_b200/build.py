@@ -24,7 +24,7 @@ CPLX_DIMS = range(1, 9)
 JIT_NX = (4, 8, 12)
 P_VEGAS = int(os.environ.get("FXJ_P_VEGAS", "1"))   # points per pass of the native Vegas kernels (fx_kernels.h)
 # resident blocks per SM the native complex kernels are held to (register budget 65536 / (128 * blocks))
-CPLX_BLOCKS = {1: 6, 2: 6, 3: 5, 4: 4, 5: 3, 6: 3, 7: 2, 8: 2}
+CPLX_BLOCKS = {1: 6, 2: 6, 3: 5, 4: 5, 5: 4, 6: 4, 7: 3, 8: 3}
 
 
 def _deps():

@@ -563,7 +563,10 @@ struct Lowering {
           if (n > 0) return Poly{};
           return Poly{Term{INFINITY, {}}};
         }
-        if (p.size() == 1 && n > 0) {
+        bool small = true;  // a monomial stays a monomial while its exponents are small; p[x[1],1000] goes
+        if (p.size() == 1)   // through L_POWI (square and multiply) instead of 999 multiplications
+          for (auto &fe : p[0].f) small = small && (long)fe.second * n <= 8;
+        if (p.size() == 1 && n > 0 && small) {
           Term t = p[0];
           double c = t.c;
           for (int i = 1; i < n; ++i) c *= t.c;  // repeated multiplication (R9)

@@ -146,8 +146,11 @@ __device__ __forceinline__ void fx_run(const fx_ins *prog, T (&X)[NX][P], const 
       FX_PLOOP { R[p] = A[p]; }
       fx_reg_dyn<T, NX, P>(op - FX_RDIV_R, X, S, R);
       fx_unpack(A, fx_slow_div(fx_pack<T, P>(R), fx_pack<T, P>(A)));
+    } else if (op == FX_END) {
+      return;
     } else {
-      return;  // FX_END (or an opcode naming a variable this kernel does not have)
+      __trap();  // an opcode this kernel has no handler for (compiler / interpreter mismatch, or a variable
+                 // index >= NX): fail loudly (the launch reports an error) instead of dropping outputs
     }
   }
 }

@@ -94,7 +94,7 @@ constexpr int FXJ_RULE = FXJ_MODE;
 // resident blocks per SM the register allocation is held to: the most for which the assembler reports
 // no spill on the configurations' programs (lattice: 6 x 80 registers at NX <= 8; plain MC carries
 // the Philox state on top: 5 x 96; Vegas also the bins and h2: 4 x 128)
-constexpr int FXJ_BLOCKS = FXJ_MODE == 2 ? (FXJ_P_VEGAS == 1 ? 6 : 4) : FXJ_MODE == 1 ? (FXJ_NX <= 8 ? 5 : 4) : (FXJ_NX <= 8 ? 6 : 4);
+constexpr int FXJ_BLOCKS = FXJ_MODE == 2 ? (FXJ_P_VEGAS == 1 ? 7 : 4) : FXJ_MODE == 1 ? (FXJ_NX <= 8 ? 5 : 4) : (FXJ_NX <= 8 ? 6 : 4);
 
 extern "C" __global__ void __launch_bounds__(FX_THREADS, FXJ_BLOCKS)
     fxj_integrate(const __grid_constant__ fx_integrate_params prm) {

@@ -604,6 +604,17 @@ def test_constants_and_operators(fb, ctx):
     assert check_points(ctx.eval_points(prog, 0, x), ref, mag) <= 1.0
 
 
+def test_large_integer_powers(fb, ctx):
+    """p[e, n] with large n goes through square-and-multiply (40 instructions, not 999), within the per-point bar."""
+    sec = one_sector([block(2, ["1+0.001*x[1]"], "p[x[1],37]*p[f[1],1000]+p[0.999*x[2],300]-p[x[1]*x[2],9]")])
+    prog = ctx.compile([sec], 2)
+    assert prog.info[0]["n_ir_ops"] < 80
+    x = np.random.default_rng(6).random((400, 2))
+    ref, mag = oracle_values_and_magnitude(spec(sec), x)
+    for tier in (0, 1):
+        assert check_points(ctx.eval_points(prog, 0, x, tier=tier), ref, mag) <= 1.0
+
+
 def test_nonfinite_is_reported(fb, ctx):
     """R13: l[e] with e <= 0 in real mode is NaN, counted, and raises FIESTA_E_NONFINITE."""
     prog = ctx.compile([one_sector([block(1, [], "l[x[1]-0.5]")])], 1)
