@@ -444,13 +444,13 @@ def run_b200(args):
             px = ctx.compile(wx.sectors, wx.dim)
             nn = px.wait_native(wx.rule)
             tcx = time.perf_counter() - t0
-            sm, km, ln, tr = timer.run(px, wx, rx, 1, 2)
+            sm, km, ln, tr = timer.run(px, wx, rx, 2, 2)
             rr = ctx.fetch_results(len(wx.sectors), wx.K)
             okx = bool(np.all(np.isfinite(rr["re"])) and np.all(rr["n_nonfinite"] == 0))
             rf = roofline_of(wx, px, len(wx.sectors), km, peak_live, tr)
             extra[name] = {"workload": f"BASELINE config {name[1]} ({name}), full size: " + describe(wx, len(wx.sectors)),
                            "value": wx.evals / (sum(sm) / len(sm) * 1e-3), "unit": UNIT, "ms_per_step": sum(sm) / len(sm),
-                           "steps": 2, "warmup": 1, "native_sectors": nn, "compile_and_assemble_s": tcx,
+                           "steps": 2, "warmup": 2, "native_sectors": nn, "compile_and_assemble_s": tcx,
                            "results_ok": okx, "gpu_launches": ln, "roofline": rf,
                            "assembler_report": px.native(0, wx.rule)[1].replace("\n", " ")[:400]}
             px.close()

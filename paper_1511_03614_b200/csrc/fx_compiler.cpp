@@ -31,6 +31,9 @@ namespace {
 #ifndef FX_HORNER_LOOK
 #define FX_HORNER_LOOK 1
 #endif
+#ifndef FX_HORNER_CAND
+#define FX_HORNER_CAND 4
+#endif
 
 [[noreturn]] void fail(int code, const std::string &msg) { throw CompileError{code, msg}; }
 
@@ -956,20 +959,23 @@ struct Emitter {
     if (q.size() == 1) return cost(r, -1, lk) + cost(q, -1, 0) + 1.0;  // monomial q: muls, then the fold with an immediate
     return cost(r, -1, lk) + cost(q, -1, lk) + 1.5;
   }
-  // every atom that divides at least two terms is tried as the variable to factor out
+  // the FX_HORNER_CAND atoms that divide most terms are tried as the variable to factor out
   static std::pair<int, double> best_variable(const Poly &terms, int look) {
     std::map<int, int> cnt;
     for (auto &t : terms)
       for (auto &fe : t.f) cnt[fe.first]++;
-    int best_v = -1, best_n = 0;
+    std::vector<std::pair<int, int>> cand;  // (-count, atom): most frequent first, ties by atom id
+    for (auto &kv : cnt) cand.push_back({-kv.second, kv.first});
+    std::sort(cand.begin(), cand.end());
+    if (terms.size() <= 3 || cand.size() == 1) return {cand[0].second, 0.0};
+    int best_v = -1;
     double best_c = 0.0;
-    for (auto &kv : cnt) {
-      if (kv.second < 2 && best_v >= 0 && best_n >= 2) continue;
-      const double c = cost(terms, kv.first, look);
-      if (best_v < 0 || c < best_c - 1e-9 || (c < best_c + 1e-9 && kv.second > best_n)) {
-        best_v = kv.first;
+    for (size_t i = 0; i < cand.size() && i < FX_HORNER_CAND; ++i) {
+      if (-cand[i].first < 2 && i > 0) break;
+      const double c = cost(terms, cand[i].second, look);
+      if (best_v < 0 || c < best_c - 1e-9) {
+        best_v = cand[i].second;
         best_c = c;
-        best_n = kv.second;
       }
     }
     return {best_v, best_c};
