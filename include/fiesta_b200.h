@@ -221,6 +221,41 @@ int fiesta_vegas_refine(fiesta_ctx *ctx, int32_t ngrids, int32_t nbins, double a
 int fiesta_vegas_grid(fiesta_ctx *ctx, int32_t sector, int32_t dim, int32_t nbins, double *grid_host,
                       double *hist_host);
 
+/* ---- contour deformation: -testF and the choice of lambda ---------------- */
+
+/* What the F(z) of a deformed sector does at sampled points. */
+typedef struct {
+  uint64_t n_points;  /* points looked at                                                            */
+  uint64_t n_bad;     /* of which Im F(z) >= 0 (or NaN): the deformation is on the wrong side there  */
+  double max_im_f;    /* max Im F(z) over the points (< 0 when n_bad == 0)                           */
+  double min_abs_f;   /* min |F(z)|: how close the contour comes to a zero of F                      */
+  double lambda;      /* the lambda this was evaluated with                                          */
+} fiesta_testf_result;
+
+/* "-testF: instead of the integration, the code checks whether the sign of the imaginary part of F is
+ * negative".  Evaluates F(z(x)) -- F = f[deform_f_index] of the sector -- at the points
+ * of `rule` (lattice or MC; npoints, seed as in fiesta_integrate), deformed with `lambda` (< 0: the
+ * sector's own), on the device.  FIESTA_E_ARG if the sector has no deformation. */
+int fiesta_test_f(fiesta_ctx *ctx, const fiesta_program *prog, int32_t sector, int32_t dim, uint64_t npoints,
+                  const fiesta_rule *rule, uint64_t seed, double lambda, fiesta_testf_result *out_host);
+
+/* The deformation size "is tuned automatically in the interval from zero to MaxComplexShift" with
+ * LambdaSplit candidates and LambdaIterations sampling points; ConservativeComplexShift halves the
+ * result.  The paper does not give the search (it defers to the FIESTA 3 paper);
+ * DESIGN.md R19: candidates lambda_max * i / lambda_split, i = 1..lambda_split, each tested with
+ * fiesta_test_f on the same `npoints` Philox points; admissible = no point with Im F(z) >= 0; the
+ * admissible candidate with the largest min |F(z)| wins (the contour that stays furthest from the
+ * zeros of F), halved if `conservative`.  scan_host (may be NULL) receives the lambda_split test
+ * results.  FIESTA_E_RULE (lambda 0) if no candidate is admissible.  The choice is returned, not
+ * applied: fiesta_program_set_lambda does that. */
+int fiesta_select_lambda(fiesta_ctx *ctx, const fiesta_program *prog, int32_t sector, int32_t dim, uint64_t npoints,
+                         uint64_t seed, double lambda_max, int32_t lambda_split, int32_t conservative,
+                         double *lambda_host, fiesta_testf_result *scan_host);
+
+/* Change the deformation size of one sector of a compiled program (lambda is a run-time parameter of
+ * both tiers' kernels: nothing is recompiled).  Synchronises the ctx stream. */
+int fiesta_program_set_lambda(fiesta_ctx *ctx, fiesta_program *prog, int32_t sector, double lambda);
+
 /* Sum over sectors with errors combined in mean square.  Host arithmetic on
  * nsectors*K numbers; total_host[K]. */
 int fiesta_combine(const fiesta_result *per_sector_host, int32_t nsectors, int32_t K, fiesta_result *total_host);

@@ -219,3 +219,39 @@ def evaluate_deformed(prog: Program, f_index: int, lam, x, xbar=None, rdtype=LD)
     cdtype = CLD if rdtype == LD else np.complex128
     z, jac = deform(prog, f_index, lam, x, xbar, rdtype)
     return evaluate(prog, z, cdtype) * det_lu(jac)
+
+
+# ----------------------------------------------------------------------------- -testF and the choice of lambda
+
+def f_at_deformed_points(prog: Program, f_index: int, lam, x, rdtype=LD):
+    """F(z(x)) for real points x[j,:]: the deformation polynomial itself on the deformed contour."""
+    cdtype = CLD if rdtype == LD else np.complex128
+    z, _ = deform(prog, f_index, lam, x, None, rdtype)
+    return evaluate(Program(prog.nvars, [], f_polynomial_tree(prog, f_index)), z, cdtype)
+
+
+def test_f(prog: Program, f_index: int, lam, x, rdtype=LD):
+    """PAPER.md:474 (-testF): "checks whether the sign of the imaginary part of F is negative".
+    -> (number of points with Im F(z) >= 0 or NaN, max Im F(z), min |F(z)|) over the points x."""
+    fz = f_at_deformed_points(prog, f_index, lam, x, rdtype)
+    bad = int(np.sum(~(fz.imag < 0)))
+    return bad, fz.imag.max(), np.abs(fz).min()
+
+
+def select_lambda(prog: Program, f_index: int, x, lambda_max=1.0, lambda_split=4, conservative=False, rdtype=LD):
+    """DESIGN.md R19, the reading of PAPER.md:404 ("tuned automatically in the interval from zero to
+    MaxComplexShift", LambdaSplit candidates, LambdaIterations points, ConservativeComplexShift):
+    candidates lambda_max*i/lambda_split, i = 1..lambda_split, each tested on the same points x;
+    admissible = no point with Im F(z) >= 0; the admissible candidate with the largest min |F(z)| is
+    chosen (first one on ties), halved if conservative.  -> (lambda or None, [(lambda_i, bad, max_im, min_abs)])."""
+    scan = []
+    best, best_min = None, None
+    for i in range(1, lambda_split + 1):
+        lam = rdtype(lambda_max) * rdtype(i) / rdtype(lambda_split)
+        bad, mx, mn = test_f(prog, f_index, lam, x, rdtype)
+        scan.append((lam, bad, mx, mn))
+        if bad == 0 and (best is None or mn > best_min):
+            best, best_min = lam, mn
+    if best is None:
+        return None, scan
+    return (best / rdtype(2) if conservative else best), scan

@@ -36,6 +36,11 @@ class _SectorDesc(C.Structure):
                 ("is_complex", C.c_int32), ("deform_f_index", C.c_int32), ("lam", C.c_double)]
 
 
+class _TestF(C.Structure):
+    _fields_ = [("n_points", C.c_uint64), ("n_bad", C.c_uint64), ("max_im_f", C.c_double), ("min_abs_f", C.c_double),
+                ("lam", C.c_double)]
+
+
 class _Rule(C.Structure):
     _fields_ = [("kind", C.c_int32), ("n_shifts", C.c_int32), ("korobov_a", C.c_uint64),
                 ("genvec", C.POINTER(C.c_uint64)), ("periodize_r", C.c_int32), ("vegas_bins", C.c_int32),
@@ -77,6 +82,10 @@ _SIGNATURES = {
     "fiesta_vegas_iteration_tier": (C.c_int, [_VP, _VP, _I32, _I32, _U64, C.POINTER(_Rule), _U64, _I32, _I32, _VP, _VP,
                                               _VP]),
     "fiesta_fp64_peak": (C.c_int, [_VP, C.c_double, C.POINTER(C.c_double)]),
+    "fiesta_test_f": (C.c_int, [_VP, _VP, _I32, _I32, _U64, C.POINTER(_Rule), _U64, C.c_double, C.POINTER(_TestF)]),
+    "fiesta_select_lambda": (C.c_int, [_VP, _VP, _I32, _I32, _U64, _U64, C.c_double, _I32, _I32, C.POINTER(C.c_double),
+                                       C.POINTER(_TestF)]),
+    "fiesta_program_set_lambda": (C.c_int, [_VP, _VP, _I32, C.c_double]),
 }
 
 _lib = None
@@ -369,6 +378,31 @@ class Context:
         tot = np.zeros(K, dtype=RESULT_DTYPE)
         self._check(self.lib.fiesta_combine(_ptr(per_sector), S, K, _ptr(tot)))
         return tot
+
+    @staticmethod
+    def _testf_dict(t):
+        return dict(n_points=int(t.n_points), n_bad=int(t.n_bad), max_im_f=float(t.max_im_f), min_abs_f=float(t.min_abs_f),
+                    lam=float(t.lam))
+
+    def test_f(self, prog, sector, npoints, rule, seed, lam=-1.0):
+        """fiesta_test_f -> dict(n_points, n_bad, max_im_f, min_abs_f, lam)."""
+        r, keep = rule._c()
+        out = _TestF()
+        self._check(self.lib.fiesta_test_f(self.handle, prog.handle, int(sector), prog.dim, int(npoints), C.byref(r),
+                                           int(seed), float(lam), C.byref(out)))
+        return self._testf_dict(out)
+
+    def select_lambda(self, prog, sector, npoints, seed, lambda_max=1.0, lambda_split=4, conservative=False):
+        """fiesta_select_lambda -> (lambda, [test result of every candidate])."""
+        lam = C.c_double()
+        scan = (_TestF * int(lambda_split))()
+        self._check(self.lib.fiesta_select_lambda(self.handle, prog.handle, int(sector), prog.dim, int(npoints), int(seed),
+                                                  float(lambda_max), int(lambda_split), int(bool(conservative)),
+                                                  C.byref(lam), scan))
+        return lam.value, [self._testf_dict(t) for t in scan]
+
+    def set_lambda(self, prog, sector, lam):
+        self._check(self.lib.fiesta_program_set_lambda(self.handle, prog.handle, int(sector), float(lam)))
 
     def fp64_peak(self, ms_target=200.0):
         t = C.c_double()

@@ -29,6 +29,7 @@ cudaError_t fx_launch_integrate_cplx(const fx_integrate_params &prm, int nsector
 cudaError_t fx_launch_eval_real(const fx_eval_params &prm, cudaStream_t st);
 cudaError_t fx_launch_eval_cplx(const fx_eval_params &prm, cudaStream_t st);
 size_t fx_eval_cplx_smem_bytes(const fx_eval_params &prm);
+cudaError_t fx_launch_testf_cplx(const fx_integrate_params &prm, int nsectors, cudaStream_t st);
 
 namespace {
 
@@ -508,6 +509,13 @@ int fiesta_compile(fiesta_ctx *ctx, const fiesta_sector_desc *sectors, int32_t n
       arena.push_back(pad);
       sd.deform_len = (uint32_t)cs.deform.size() + 1;
     }
+    if (!cs.testf.empty()) {
+      sd.testf_off = (uint32_t)arena.size();
+      arena.insert(arena.end(), cs.testf.begin(), cs.testf.end());
+      arena.push_back(pad);
+      sd.testf_len = (uint32_t)cs.testf.size() + 1;
+    }
+    sd.n_mem_testf = cs.n_mem_testf;
     sd.K = cs.K;
     sd.is_complex = cs.is_complex ? 1 : 0;
     sd.sector_id = cs.sector_id;
@@ -656,6 +664,7 @@ int fiesta_combine(const fiesta_result *per_sector, int32_t nsectors, int32_t K,
 // dispatch of the complex kernels, one translation unit per dimension (fx_kernels_cplx.cu -DFX_N=n)
 // ------------------------------------------------------------------------------------------------
 #define FX_DECL_CPLX(n)                                                                                         \
+  cudaError_t fx_launch_testf_cplx_n##n(const fx_integrate_params &prm, int nsectors, size_t smem, cudaStream_t st); \
   cudaError_t fx_launch_integrate_cplx_n##n(const fx_integrate_params &prm, int nsectors, size_t smem, cudaStream_t st); \
   cudaError_t fx_launch_eval_cplx_n##n(const fx_eval_params &prm, size_t smem, cudaStream_t st);
 FX_DECL_CPLX(1) FX_DECL_CPLX(2) FX_DECL_CPLX(3) FX_DECL_CPLX(4) FX_DECL_CPLX(5) FX_DECL_CPLX(6) FX_DECL_CPLX(7) FX_DECL_CPLX(8)
@@ -678,6 +687,16 @@ cudaError_t fx_launch_eval_cplx(const fx_eval_params &prm, cudaStream_t st) {
   const size_t smem = fx_eval_cplx_smem_bytes(prm);
   switch (prm.dim) {
 #define FX_CASE(n) case n: return fx_launch_eval_cplx_n##n(prm, smem, st);
+    FX_CASE(1) FX_CASE(2) FX_CASE(3) FX_CASE(4) FX_CASE(5) FX_CASE(6) FX_CASE(7) FX_CASE(8)
+#undef FX_CASE
+  }
+  return cudaErrorInvalidValue;
+}
+
+cudaError_t fx_launch_testf_cplx(const fx_integrate_params &prm, int nsectors, cudaStream_t st) {
+  const size_t smem = fx_integrate_smem_bytes(prm);
+  switch (prm.dim) {
+#define FX_CASE(n) case n: return fx_launch_testf_cplx_n##n(prm, nsectors, smem, st);
     FX_CASE(1) FX_CASE(2) FX_CASE(3) FX_CASE(4) FX_CASE(5) FX_CASE(6) FX_CASE(7) FX_CASE(8)
 #undef FX_CASE
   }

@@ -1284,6 +1284,20 @@ CompiledSector compile_sector(const char *const *texts, int K, int dim, bool is_
     cs.deform = em.code;
     cs.n_mem_deform = em.mhigh;
     cs.info.n_deform_ops = (int)cs.deform.size() - 1;
+    {  // F itself as a one-output complex program: what -testF evaluates at the deformed points
+      Lowering lowf(raw, fbound, dim);
+      lowf.cplx = true;
+      const int rootf = lowf.lower(funcs0[deform_f_index - 1]);
+      Emitter ef(lowf.nodes, dim, 0);
+      ef.count_uses(rootf);
+      for (auto &n : lowf.nodes) n.rem = n.uses;
+      ef.value_to_a(rootf);
+      ef.consume(rootf);
+      ef.ins(FX_OUT, 0);
+      ef.ins(FX_END);
+      cs.testf = ef.code;
+      cs.n_mem_testf = ef.mhigh;
+    }
     fiesta_compile_info di{};
     fill_info(cs.deform, di, false);
     cs.info.flops += di.flops;

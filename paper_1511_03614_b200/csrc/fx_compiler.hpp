@@ -18,6 +18,7 @@ struct CompileError {
 struct CompiledSector {
   std::vector<fx_ins> main;    // K outputs through FX_OUT, ends with FX_END
   std::vector<fx_ins> deform;  // gradient/Hessian of F through FX_STM, ends with FX_END; empty if none
+  std::vector<fx_ins> testf;   // deformed sectors: complex program with the single output F(z) (PAPER.md:474 -testF)
   int K = 0;
   int dim = 0;
   int sector_id = 0;
@@ -26,6 +27,7 @@ struct CompiledSector {
   double lambda = 0.0;
   int n_mem_main = 0;    // M slots (scalars of the program's arithmetic type) of the main program
   int n_mem_deform = 0;  // M slots (doubles) of the deformation program, outputs included
+  int n_mem_testf = 0;   // M slots (complex) of the F(z) program
   fiesta_compile_info info{};
 };
 

@@ -23,8 +23,10 @@ struct fx_sector_dev {       // one compiled sector in the device arena
   int32_t sector_id;
   int32_t n_mem_main;        // spill slots (scalars of the program's type)
   int32_t n_mem_deform;      // spill slots (doubles) incl. the gradient/Hessian outputs
-  int32_t pad;
+  int32_t n_mem_testf;       // spill slots (complex) of the F(z) program
   double lambda;
+  uint32_t testf_off;        // F(z) program of a deformed sector (fiesta_test_f); 0 length: none
+  uint32_t testf_len;
 };
 
 struct fx_transform_host {
@@ -65,7 +67,9 @@ struct fx_integrate_params {
   const int32_t *launch_map;
   int32_t sel_base;
   int32_t batch_base;        // position in the selection of the batch's first sector
-  unsigned long long *testf; // [nsel]: points with Im F(z) >= 0 (deformed sectors; PAPER.md:474 -testF), or NULL
+  // fiesta_test_f (PAPER.md:474 -testF): one record per block, [bad points, max Im F(z), min |F(z)|^2, points]
+  double *testf_out;
+  double lambda_override;    // >= 0: use instead of the sector's lambda (the lambda scan); < 0: the sector's own
 };
 
 // position in the selection of the sector a block works on

@@ -143,6 +143,86 @@ __global__ void __launch_bounds__(FX_THREADS) fx_integrate_cplx(const __grid_con
   fx_block_finish(prm, N, sel_idx, chunk, nonfinite, sh_hist);
 }
 
+// -testF: "instead of the integration, the code checks whether the sign of the imaginary
+// part of F is negative".  The sector's F(z) program is walked at the rule's points, deformed with
+// lambda (the sector's, or the candidate of a lambda scan); per block one record:
+// points with Im F(z) >= 0 (or NaN), max Im F(z), min |F(z)|^2, points looked at.
+struct TestFSink {
+  unsigned valid;
+  unsigned bad;
+  double max_im, min_abs2;
+  __device__ __forceinline__ void operator()(int, cplx (&A)[P]) {
+    FX_PLOOP {
+      if ((valid >> p) & 1u) {
+        bad += (A[p].im < 0.0) ? 0u : 1u;
+        max_im = fmax(max_im, A[p].im);
+        min_abs2 = fmin(min_abs2, fma(A[p].re, A[p].re, A[p].im * A[p].im));
+      }
+    }
+  }
+};
+
+template <int RULE>
+__global__ void __launch_bounds__(FX_THREADS) fx_testf_cplx(const __grid_constant__ fx_integrate_params prm) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  const int b = blockIdx.x;
+  const int chunk = b % prm.nchunks;
+  const int r = (b / prm.nchunks) % prm.n_shifts;
+  const int sel_idx = fx_sel_index(prm, b / (prm.nchunks * prm.n_shifts));
+  const fx_sector_dev sec = prm.sectors[prm.sel[sel_idx]];
+  const fx_smem_layout L = fx_layout(prm.prog_ins_max, prm.mem_doubles, N, prm.nbins, false);
+  fx_ins *sh_prog = reinterpret_cast<fx_ins *>(smem + L.prog);
+  fx_ins *sh_deform = sh_prog + sec.testf_len;
+  double *sh_mem = reinterpret_cast<double *>(smem + L.mem);
+  uint64_t *sh_delta = reinterpret_cast<uint64_t *>(smem + L.delta);
+  double *sh_red = reinterpret_cast<double *>(smem + L.acc);
+  fx_copy_program(sh_prog, prm.arena + sec.testf_off, sec.testf_len);
+  fx_copy_program(sh_deform, prm.arena + sec.deform_off, sec.deform_len);
+  fx_block_setup(prm, N, (uint32_t)sec.sector_id, r, sel_idx, sh_delta, nullptr, nullptr);
+  __syncthreads();
+  const double lambda = prm.lambda_override >= 0.0 ? prm.lambda_override : sec.lambda;
+  const uint64_t c0 = (uint64_t)chunk * prm.chunk;
+  const uint64_t c1 = min(c0 + prm.chunk, prm.n_per_shift);
+  const fx_mem<double> Mr{sh_mem + threadIdx.x, FX_THREADS};
+  const fx_mem<cplx> Mc{sh_mem + threadIdx.x, FX_THREADS};
+  TestFSink sink{0u, 0u, -INFINITY, INFINITY};
+  unsigned seen = 0;
+  for (uint64_t base = c0 + (uint64_t)threadIdx.x * P; base < c1; base += (uint64_t)FX_THREADS * P) {
+    double x[N][P], xbar[N][P], W[P];
+    uint32_t bins[(N + 3) / 4][P];
+    unsigned valid;
+    fx_make_points<RULE, N, P, true>(prm, N, (uint32_t)sec.sector_id, sh_delta, nullptr, base, c1, x, xbar, W, valid, bins);
+    cplx X[N][P], det[P];
+    fx_deform_points(sh_deform, lambda, x, xbar, Mr, X, det);
+    sink.valid = valid;
+    seen += __popc(valid);
+    fx_run<cplx, N, P>(sh_prog, X, Mc, sink);
+  }
+  // block reduction in a fixed order: lanes by shuffle tree, warps in order
+  double v[4] = {(double)sink.bad, sink.max_im, sink.min_abs2, (double)seen};
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) {
+    v[0] += __shfl_down_sync(0xffffffffu, v[0], off);
+    v[1] = fmax(v[1], __shfl_down_sync(0xffffffffu, v[1], off));
+    v[2] = fmin(v[2], __shfl_down_sync(0xffffffffu, v[2], off));
+    v[3] += __shfl_down_sync(0xffffffffu, v[3], off);
+  }
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0)
+    for (int q = 0; q < 4; ++q) sh_red[(threadIdx.x >> 5) * 4 + q] = v[q];
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double o[4] = {0.0, -INFINITY, INFINITY, 0.0};
+    for (int w = 0; w < FX_THREADS / 32; ++w) {
+      o[0] += sh_red[w * 4];
+      o[1] = fmax(o[1], sh_red[w * 4 + 1]);
+      o[2] = fmin(o[2], sh_red[w * 4 + 2]);
+      o[3] += sh_red[w * 4 + 3];
+    }
+    for (int q = 0; q < 4; ++q) prm.testf_out[(size_t)b * 4 + q] = o[q];
+  }
+}
+
 struct EvalSinkCplx {
   double *out;
   int K;
@@ -216,5 +296,20 @@ cudaError_t FX_CAT(fx_launch_eval_cplx_n, FX_N)(const fx_eval_params &prm, size_
   const unsigned grid = (unsigned)((prm.npts + per_block - 1) / per_block);
   if (grid == 0) return cudaSuccess;
   fx_eval_cplx<<<grid, FX_THREADS, smem, st>>>(prm);
+  return cudaGetLastError();
+}
+
+cudaError_t FX_CAT(fx_launch_testf_cplx_n, FX_N)(const fx_integrate_params &prm, int nsectors, size_t smem, cudaStream_t st) {
+  const unsigned grid = (unsigned)((size_t)nsectors * prm.n_shifts * prm.nchunks);
+  cudaError_t e;
+#define FX_LAUNCH(RULE)                                                                                            \
+  {                                                                                                                \
+    e = cudaFuncSetAttribute(fx_testf_cplx<RULE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);         \
+    if (e != cudaSuccess) return e;                                                                                \
+    fx_testf_cplx<RULE><<<grid, FX_THREADS, smem, st>>>(prm);                                                        \
+  }
+  if (prm.rule == FIESTA_RULE_LATTICE) FX_LAUNCH(FIESTA_RULE_LATTICE)
+  else FX_LAUNCH(FIESTA_RULE_MC)
+#undef FX_LAUNCH
   return cudaGetLastError();
 }

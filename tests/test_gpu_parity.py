@@ -447,6 +447,65 @@ def test_lambda_zero_reproduces_real_path(fb, ctx):
     assert np.allclose(b.real[ok], a.real[ok], rtol=1e-11) and np.all(np.abs(b.imag[ok]) <= 1e-11 * np.abs(a.real[ok]))
 
 
+# ------------------------------------------------------------------------------ -testF, choice of lambda
+
+def test_testf_and_lambda_scan(fb, ctx):
+    """PAPER.md:474 -testF and the automatic deformation size of PAPER.md:404 (R19) on the device
+    against the oracle: counts of points with Im F(z) >= 0 bit-exact, max Im F and min |F| to 1e-12; the scan
+    picks the same candidate; fiesta_program_set_lambda changes what both tiers integrate."""
+    from oracle import deform as OD
+    from oracle.parser import parse
+    wl = make_workload("C4", nsectors=2, npoints=1 << 12)
+    cub = one_sector([block(1, ["p[x[1],3]-0.2"], "1/f[1]")], sector_id=9, is_complex=True, deform_f_index=1, lam=1.0)
+    prog = ctx.compile(wl.sectors, wl.dim)
+    mc = fb.Rule(kind=fb.RULE_MC)
+    for si, lam in ((0, -1.0), (1, 0.25), (1, 6.0), (0, 40.0)):
+        s = wl.sectors[si]
+        sec = spec(s)
+        _, x = OI.mc_points(sec, 77, 0, 0, 3001)
+        lam_o = s.lam if lam < 0 else lam
+        bad, mx, mn = OD.test_f(sec.progs[0], s.deform_f_index, lam_o, x)
+        got = ctx.test_f(prog, si, 3001, mc, 77, lam)
+        assert got["n_points"] == 3001 and got["lam"] == lam_o
+        assert got["n_bad"] == bad, (si, lam, got, bad)
+        assert abs(got["max_im_f"] - float(mx)) <= 1e-12 * max(abs(float(mx)), 1.0)
+        assert abs(got["min_abs_f"] - float(mn)) <= 1e-12 * float(mn)
+    assert ctx.test_f(prog, 0, 3001, mc, 77)["n_bad"] == 0          # the generator rejected seeds with Im F >= 0
+    # lattice points as well
+    rule = fb.Rule(kind=fb.RULE_LATTICE, n_shifts=2, korobov_a=wl.korobov_a, periodize_r=3)
+    got = ctx.test_f(prog, 1, 1 << 12, rule, 5, 0.5)
+    sec = spec(wl.sectors[1])
+    # the Korobov vector the rule above implies for its 2^11-point lattice: a^k mod 2^11
+    gv = OP.korobov_genvec(wl.korobov_a, 1 << 11, wl.dim)
+    xs = np.concatenate([OI.lattice_points(sec, 1 << 11, gv, 3, 5, r, 0, 1 << 11)[0] for r in range(2)])
+    bad, mx, mn = OD.test_f(sec.progs[0], 2, 0.5, xs)
+    assert got["n_bad"] == bad and abs(got["min_abs_f"] - float(mn)) <= 1e-12 * float(mn)
+    # the scan on the 1-D cubic, whose admissible range is known in closed form (lam < 3.897..)
+    p1 = ctx.compile([cub], 1)
+    secc = spec(cub)
+    _, x = OI.mc_points(secc, 123, (1 << 20) - 1, 0, 1000)
+    lam_o, scan_o = OD.select_lambda(secc.progs[0], 1, x, lambda_max=8.0, lambda_split=8)
+    lam_g, scan_g = ctx.select_lambda(p1, 0, 1000, 123, lambda_max=8.0, lambda_split=8)
+    assert lam_g == float(lam_o) and [t["n_bad"] for t in scan_g] == [t[1] for t in scan_o]
+    assert [t["n_bad"] == 0 for t in scan_g] == [True, True, True] + [False] * 5
+    assert ctx.select_lambda(p1, 0, 1000, 123, 8.0, 8, conservative=True)[0] == lam_g / 2
+    with pytest.raises(fb.FiestaError) as ei:
+        ctx.select_lambda(p1, 0, 1000, 123, lambda_max=80.0, lambda_split=2)
+    assert ei.value.code == -4
+    # applying the choice: a run-time parameter of both tiers
+    lat = fb.Rule(kind=fb.RULE_LATTICE, n_shifts=2, korobov_a=1, periodize_r=3)
+    before = ctx.integrate(p1, 1 << 12, lat, 3, tier=fb.TIER_NATIVE)
+    ctx.set_lambda(p1, 0, lam_g)
+    a = ctx.integrate(p1, 1 << 12, lat, 3, tier=fb.TIER_NATIVE)
+    b = ctx.integrate(p1, 1 << 12, lat, 3, tier=fb.TIER_INTERPRETER)
+    assert a.tobytes() == b.tobytes() and a.tobytes() != before.tobytes()
+    val, sig = OI.integrate_lattice(SectorSpec(cub.texts, 9, True, 1, lam_g), 1 << 12, 2, [1], 3, 3)
+    assert np.allclose(a[0]["re"], np.asarray(val, dtype=float)[:, 0], rtol=1e-9)
+    assert np.allclose(a[0]["im"], np.asarray(val, dtype=float)[:, 1], rtol=1e-9)
+    with pytest.raises(fb.FiestaError):
+        ctx.test_f(ctx.compile(make_workload("C1", nsectors=1, npoints=1 << 12).sectors, 4), 0, 100, mc, 1)
+
+
 # ------------------------------------------------------------------------------ A3/A8: Vegas
 
 def _c5(nsec, npts):

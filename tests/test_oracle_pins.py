@@ -13,7 +13,7 @@ import scipy.special
 from conftest import golden
 from oracle import points as P
 from oracle.deform import (deform, det_lu, differentiate, evaluate_deformed, f_polynomial_tree,
-                           gradient_and_hessian)
+                           gradient_and_hessian, select_lambda, test_f as oracle_test_f)
 from oracle.evaluate import CLD, LD, evaluate, evaluate_with_magnitude, polygamma_const, PI, EULER_GAMMA
 from oracle.integrate import (SectorSpec, combine_sectors, estimate_from_sums, integrate_lattice, integrate_mc,
                               integrate_vegas, lattice_partial_sums, neumaier_sum, vegas_combine, vegas_refine,
@@ -695,3 +695,36 @@ def test_fp64_horner_of_phi_r_errs_by_its_condition_number():
         assert rel.max() < (2.0e-15 if r <= 4 else 2.0e-14)
         # r = 5, 6 do need the wider bar: the polynomial's own error is already above 4e-15
         assert (rel.max() > 4e-15) == (r >= 5)
+
+
+def test_testf_and_lambda_selection_closed_forms():
+    """PAPER.md:474 (-testF), :404 (lambda tuned in (0, MaxComplexShift]); R19.  1-D closed forms:
+    F = x - a:   F(z) = (x - a) - i lam x(1-x): Im F < 0 for every lam > 0, |F|^2 = (x-a)^2 + lam^2 s^2 grows
+                 with lam, so the scan picks lambda_max;
+    F = x^3 - a: z = x - i lam s 3x^2, Im F(z) = lam s g (lam^2 s^2 g^2 - 3 x^2), g = 3x^2, s = x(1-x): the
+                 point x is bad exactly when lam s g >= sqrt(3) x, i.e. lam >= 1/(sqrt(3) x^2 (1-x))."""
+    rng = np.random.default_rng(21)
+    x = rng.uniform(0.02, 0.98, size=(4000, 1)).astype(LD)
+    xs = x[:, 0]
+    lin = parse(block(1, ["x[1]-0.3"], "1/f[1]"))
+    for lam in (0.1, 0.5, 3.0):
+        bad, mx, mn = oracle_test_f(lin, 1, lam, x)
+        s = xs * (1 - xs)
+        assert bad == 0
+        assert abs(float(mx - np.max(-LD(lam) * s))) < 1e-18
+        assert abs(float(mn - np.min(np.sqrt((xs - LD(0.3)) ** 2 + (LD(lam) * s) ** 2)))) < 1e-18
+    lam, scan = select_lambda(lin, 1, x, lambda_max=2.0, lambda_split=4)
+    assert float(lam) == 2.0 and [float(t[0]) for t in scan] == [0.5, 1.0, 1.5, 2.0] and all(t[1] == 0 for t in scan)
+    assert float(select_lambda(lin, 1, x, 2.0, 4, conservative=True)[0]) == 1.0
+    cub = parse(block(1, ["p[x[1],3]-0.2"], "1/f[1]"))
+    thr = 1 / (np.sqrt(LD(3)) * xs ** 2 * (1 - xs))               # lam at which the point turns bad
+    for lam in (1.0, 4.0, 6.0, 9.0):
+        bad, mx, mn = oracle_test_f(cub, 1, lam, x)
+        assert bad == int(np.sum(thr <= LD(lam)))
+    assert oracle_test_f(cub, 1, 3.85, x)[0] == 0 and oracle_test_f(cub, 1, 4.0, x)[0] > 0    # min thr = 27/(4 sqrt 3) = 3.897.. at x = 2/3
+    lam, scan = select_lambda(cub, 1, x, lambda_max=8.0, lambda_split=8)
+    ok = [t for t in scan if t[1] == 0]
+    assert [float(t[0]) for t in ok] == [1.0, 2.0, 3.0]            # the candidates below 3.897
+    assert float(lam) == float(max(ok, key=lambda t: t[3])[0])
+    none, scan = select_lambda(cub, 1, x, lambda_max=80.0, lambda_split=2)
+    assert none is None and all(t[1] > 0 for t in scan)
