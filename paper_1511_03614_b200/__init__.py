@@ -11,4 +11,6 @@ from .binding import (  # noqa: F401
     RESULT_DTYPE, INFO_DTYPE,
 )
 
+from .pool import IntegrationPool, ResultStore  # noqa: F401,E402
+
 load = load_library

@@ -801,6 +801,27 @@ def test_c5_full_size_one_iteration(fb, ctx):
     assert np.allclose(h.sum(axis=1), sums[0, 0, 1], rtol=1e-12)
 
 
+def test_integration_pool_on_the_gpu(fb, ctx, tmp_path):
+    """The queue of paper_1511_03614_b200/pool.py around the real C ABI: groups compiled one
+    ahead, results stored per (sector, order), a killed job resumed -- the same bits as one fiesta_integrate call."""
+    from paper_1511_03614_b200.pool import IntegrationPool
+    wl = make_workload("C2", nsectors=20, npoints=1 << 14)
+    rule = fb.Rule.from_workload(wl)
+    prog = ctx.compile(wl.sectors, wl.dim)
+    direct = ctx.integrate(prog, wl.npoints, rule, wl.seed)
+    path = str(tmp_path / "results.db")
+    costs = [s.naive_ops for s in wl.sectors]
+    pool = IntegrationPool(ctx, wl.sectors, wl.dim, rule, wl.npoints, wl.seed, store_path=path, group=6, costs=costs)
+    assert not pool.run(max_groups=2) and pool.n_integrated == 12
+    pool = IntegrationPool(ctx, wl.sectors, wl.dim, rule, wl.npoints, wl.seed, store_path=path, group=6, costs=costs)
+    assert pool.run() and pool.n_from_store == 12 and pool.n_integrated == 8
+    res = pool.results()
+    for f in ("re", "re_err", "neval"):            # JSON keeps every bit of a double
+        assert np.array_equal(res[f], direct[f])
+    tot = pool.totals()
+    assert np.array_equal(tot["re"], ctx.combine(direct)["re"]) and np.array_equal(tot["re_err"], ctx.combine(direct)["re_err"])
+
+
 def test_fp64_peak_is_plausible(ctx):
     """The roofline denominator: DFMA streams on every SM.  B200: 148 SM x 64 lanes x 2 x 1.965 GHz = 37.2."""
     t = ctx.fp64_peak(50.0)

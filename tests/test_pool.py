@@ -1,0 +1,157 @@
+"""CPU tests of the integration pool (paper_1511_03614_b200/pool.py): queue, partition, restartable store,
+-part, totals; world size 2 over gloo.  The GPU is replaced by a stand-in context that returns numbers which
+depend on the sector only; the GPU test of the pool is in test_gpu_parity.py."""
+import os
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+_FAKE = r"""
+import numpy as np
+from dataclasses import dataclass, field
+from paper_1511_03614_b200.binding import RESULT_DTYPE, Rule
+
+@dataclass
+class Sec:
+    sector_id: int
+    texts: list
+    is_complex: bool = False
+    deform_f_index: int = 0
+    lam: float = 0.0
+
+class FakeProg:
+    def __init__(self, sectors): self.sectors, self.closed = sectors, False
+    def close(self): self.closed = True
+
+class FakeCtx:
+    '''Stands in for binding.Context: the value of (sector, order) is a fixed function of the sector id.'''
+    def __init__(self): self.compiled, self.integrated = [], []
+    def compile(self, sectors, dim):
+        self.compiled.append([s.sector_id for s in sectors]); return FakeProg(sectors)
+    def integrate(self, prog, npoints, rule, seed, allow_nonfinite=False):
+        assert not prog.closed
+        out = np.zeros((len(prog.sectors), len(prog.sectors[0].texts)), dtype=RESULT_DTYPE)
+        for i, s in enumerate(prog.sectors):
+            for k in range(out.shape[1]):
+                out[i, k] = (s.sector_id + 0.25 * k, 0.5 + s.sector_id, -k, 0.0, 0.0, npoints, 0)
+        self.integrated.append([s.sector_id for s in prog.sectors]); return out
+
+def sectors(n, K=2):
+    return [Sec(100 + i, ["1;\n0;\nx[1]+%d.%d;\n|" % (i, k) for k in range(K)]) for i in range(n)]
+"""
+
+
+def _ns():
+    ns = {}
+    sys.path.insert(0, ROOT)
+    exec(_FAKE, ns)
+    return ns
+
+
+def test_pool_queue_store_and_resume(tmp_path, lib):
+    from paper_1511_03614_b200.pool import IntegrationPool, ResultStore
+    ns = _ns()
+    secs, rule = ns["sectors"](23), ns["Rule"](kind=1)
+    costs = [(i * 7) % 5 + 1 for i in range(23)]
+    path = str(tmp_path / "out.db")
+    ctx = ns["FakeCtx"]()
+    pool = IntegrationPool(ctx, secs, 1, rule, 1000, 7, store_path=path, group=5, costs=costs)
+    assert not pool.run(max_groups=2)                       # a time limit: two groups of five, largest first
+    assert pool.n_integrated == 10 and len(ctx.integrated) == 2
+    assert all(costs[s - 100] >= 3 for g in ctx.integrated for s in g) and ctx.integrated[0] == [102, 107, 112, 117, 122]
+    assert ctx.compiled == ctx.integrated                   # group 2 was handed to the compiler before group 1 ran; none beyond the limit
+    with pytest.raises(RuntimeError):
+        pool.totals()
+    with open(path + ".rank0", "a") as fh:                  # the job was killed in the middle of a write
+        fh.write('{"sig": "torn')
+    # a new process continues from where it stopped: only the missing 13 are integrated
+    ctx2 = ns["FakeCtx"]()
+    pool2 = IntegrationPool(ctx2, secs, 1, rule, 1000, 7, store_path=path, group=5, costs=costs)
+    assert pool2.run() and pool2.n_from_store == 10 and pool2.n_integrated == 13
+    done_before = {s for g in ctx.integrated for s in g}
+    assert not done_before & {s for g in ctx2.integrated for s in g}
+    res = pool2.results()
+    assert res.shape == (23, 2)
+    for i in range(23):
+        assert res[i, 1]["re"] == 100 + i + 0.25 and res[i, 0]["neval"] == 1000
+    tot = pool2.totals()
+    assert tot[0]["re"] == sum(100 + i for i in range(23))
+    assert abs(tot[1]["re_err"] - np.sqrt(sum((0.5 + 100 + i) ** 2 for i in range(23)))) < 1e-9
+    # other points / seed / texts: another signature, nothing is reused
+    pool3 = IntegrationPool(ns["FakeCtx"](), secs, 1, rule, 2000, 7, store_path=path, group=50, costs=costs)
+    assert len(pool3.pending()) == 23
+    # a third run finds everything there and launches nothing
+    ctx4 = ns["FakeCtx"]()
+    pool4 = IntegrationPool(ctx4, secs, 1, rule, 1000, 7, store_path=path, group=5, costs=costs)
+    assert pool4.run() and ctx4.integrated == [] and pool4.totals().tobytes() == tot.tobytes()
+
+
+def test_pool_part_option(tmp_path, lib):
+    """-part i/n: the parts are disjoint, cover everything, and their totals add up."""
+    from paper_1511_03614_b200.pool import IntegrationPool
+    ns = _ns()
+    secs, rule = ns["sectors"](10), ns["Rule"](kind=1)
+    seen, total = [], 0.0
+    for i in (1, 2, 3):
+        ctx = ns["FakeCtx"]()
+        pool = IntegrationPool(ctx, secs, 1, rule, 500, 1, group=4, part=(i, 3))
+        assert pool.run()
+        seen += [s for g in ctx.integrated for s in g]
+        total += pool.totals()[0]["re"]
+    assert sorted(seen) == [100 + i for i in range(10)] and total == sum(100 + i for i in range(10))
+    with pytest.raises(ValueError):
+        IntegrationPool(ns["FakeCtx"](), secs, 1, rule, 500, 1, part=(4, 3))
+
+
+_GLOO_POOL = r"""
+import os, sys
+import numpy as np
+import torch.distributed as dist
+sys.path.insert(0, {root!r})
+exec(open({fake!r}).read())
+from paper_1511_03614_b200.pool import IntegrationPool
+dist.init_process_group("gloo", init_method="tcp://127.0.0.1:{port}", rank=int(sys.argv[1]), world_size=2)
+secs, rule = sectors(17), Rule(kind=1)
+costs = [(i * 5) % 7 + 1 for i in range(17)]
+ctx = FakeCtx()
+pool = IntegrationPool(ctx, secs, 1, rule, 1000, 3, store_path={store!r}, group=4, costs=costs, dist=dist)
+assert pool.run()
+mine = sorted(s for g in ctx.integrated for s in g)
+res = pool.results()
+assert res.shape == (17, 2) and all(res[i, 0]["re"] == 100 + i for i in range(17))
+tot = pool.totals()
+assert tot[0]["re"] == sum(100 + i for i in range(17))
+load = sum(costs[s - 100] for s in mine)
+print("ok", dist.get_rank(), len(mine), load)
+dist.barrier()
+dist.destroy_process_group()
+"""
+
+
+def test_pool_world_size_2_gloo(tmp_path):
+    fake = tmp_path / "fake.py"
+    fake.write_text(_FAKE)
+    script = tmp_path / "w.py"
+    port = 29500 + os.getpid() % 2000
+    script.write_text(_GLOO_POOL.format(root=ROOT, fake=str(fake), port=port, store=str(tmp_path / "db")))
+    procs = [subprocess.Popen([sys.executable, str(script), str(r)], stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True)
+             for r in range(2)]
+    outs = [p.communicate(timeout=180) for p in procs]
+    for p, (o, e) in zip(procs, outs):
+        assert p.returncode == 0, e[-2000:]
+    n = [int(o.split()[2]) for o, _ in outs]
+    loads = [int(o.split()[3]) for o, _ in outs]
+    assert sum(n) == 17 and abs(loads[0] - loads[1]) <= 7       # every sector once, balanced by cost
+    # both ranks wrote their own file; a single-process restart finds all 17 there
+    sys.path.insert(0, ROOT)
+    ns = {}
+    exec(_FAKE, ns)
+    from paper_1511_03614_b200.pool import IntegrationPool
+    ctx = ns["FakeCtx"]()
+    pool = IntegrationPool(ctx, ns["sectors"](17), 1, ns["Rule"](kind=1), 1000, 3, store_path=str(tmp_path / "db"), group=4,
+                           costs=[(i * 5) % 7 + 1 for i in range(17)])
+    assert pool.run() and ctx.integrated == []
