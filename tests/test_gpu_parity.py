@@ -222,6 +222,28 @@ def test_native_and_interpreter_tiers_agree_bitwise(fb, ctx, name, nsec, npts, n
     assert r1.tobytes() == r2.tobytes() == r3.tobytes()
 
 
+def test_first_call_mixes_tiers_with_identical_bits(fb, ctx):
+    """fiesta_compile returns before the native kernels exist; the first fiesta_integrate serves every sector
+    with whichever form is ready at its launch (the integrand is transformed once, then evaluated).
+    Whatever the split was, the results are the bits of an all-native and of an all-interpreter pass."""
+    wl = make_workload("C3", nsectors=48, npoints=1 << 16)
+    rule = fb.Rule.from_workload(wl)
+    prog = ctx.compile(wl.sectors, wl.dim)
+    first = ctx.integrate(prog, wl.npoints, rule, wl.seed)           # no waiting
+    n_nat, n_int = ctx.last_tiers()
+    assert n_nat + n_int == 48
+    assert prog.wait_native() == 48
+    st = prog.native_stats()
+    assert st["assembled"] + st["cache_hits"] >= 48 and st["threads"] >= 1
+    allnat = ctx.integrate(prog, wl.npoints, rule, wl.seed)
+    assert ctx.last_tiers() == (48, 0)
+    interp = ctx.integrate(prog, wl.npoints, rule, wl.seed, tier=fb.TIER_INTERPRETER)
+    assert first.tobytes() == allnat.tobytes() == interp.tobytes()
+    # the same texts again: the kernels come from the cache (keyed by the program, not the sector id)
+    prog2 = ctx.compile(wl.sectors[:8], wl.dim)
+    assert prog2.wait_native() == 8 and prog2.native_stats()["cache_hits"] == 8
+
+
 def test_native_tier_is_off_with_fiesta_jit_0(fb, ctx, monkeypatch):
     wl = make_workload("C2", nsectors=2, npoints=1 << 12)
     monkeypatch.setenv("FIESTA_JIT", "0")
