@@ -92,14 +92,18 @@ typedef struct {
  *   (2) that same sequence lowered instruction by instruction to PTX, spliced into the evaluation
  *       kernel and assembled for sm_100a in process: one native kernel per (sector, mode), mode =
  *       a FIESTA_RULE_* or FIESTA_MODE_EVAL (real and complex sectors).  The program's own
- *       background threads assemble them (~0.1-0.2 s of one host core per kernel): the lattice
- *       rule's from fiesta_compile on, another mode's from the first call that uses it on.
- * fiesta_integrate serves every sector with its native kernel if that is ready and with the
+ *       background threads assemble them (~0.1-0.2 s of one host core per kernel), from the first
+ *       call on that can use them: a call asks for the kernels of its rule for those of its
+ *       sectors whose work per pass (points x instructions) is large enough for a launch of their
+ *       own to pay (FIESTA_NATIVE_MIN_WORK, default 2e7); smaller sectors stay on the interpreter,
+ *       which takes all of them in one launch.
+ * fiesta_integrate serves every such sector with its native kernel if that is ready and with the
  * interpreter otherwise; both forms perform the same operations in the same order with the same
  * roundings, so a sector's sums are bit-identical whichever served it.
- * Environment (read at each fiesta_compile): FIESTA_JIT=0 no native tier; FIESTA_JIT=sync return
- * only when every sector's lattice kernel is ready; FIESTA_CACHE_DIR=<dir> keep assembled kernels
- * on disk, keyed by the program (a process-wide in-memory cache always exists). */
+ * Environment (read at each fiesta_compile): FIESTA_JIT=0 no native tier; FIESTA_JIT=eager queue the
+ * lattice kernels of all sectors at once; FIESTA_JIT=sync the same and return only when they are
+ * ready; FIESTA_CACHE_DIR=<dir> keep assembled kernels on disk, keyed by the program (a process-wide
+ * in-memory cache always exists). */
 int fiesta_compile(fiesta_ctx *ctx, const fiesta_sector_desc *sectors, int32_t nsectors, int32_t dim,
                    fiesta_program **out, fiesta_compile_info *info);
 void fiesta_program_free(fiesta_program *prog);

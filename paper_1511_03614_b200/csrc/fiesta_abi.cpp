@@ -154,6 +154,8 @@ struct Plan {
   int mode = 0;               // fx::JitMode of the rule
   int batch = 1;              // sectors per batch (run_pass)
   bool allow_native = true;
+  bool force_native = false;  // FIESTA_TIER_NATIVE: also for sectors below the work threshold
+  double min_work = 0.0;      // points x instructions per sector and pass from which a native launch pays
   bool uniform_K = true;
   bool any_real = false, any_cplx = false;
   int Kmax = 0;
@@ -444,11 +446,13 @@ int fiesta_compile(fiesta_ctx *ctx, const fiesta_sector_desc *sectors, int32_t n
   // sectors are independent: parse/optimise them on the host cores in parallel, then lay the
   // programs out in the arena in sector order
   std::vector<fx::CompiledSector> compiled(nsectors);
-  // FIESTA_JIT: "0" no native tier; "sync" fiesta_compile returns when every sector's lattice kernel is
-  // assembled; anything else (default) assembles in the background while the interpreter serves
+  // FIESTA_JIT: "0" no native tier; "eager" the lattice kernels of all sectors are queued for assembly
+  // here; "sync" the same, and fiesta_compile returns only when they are ready; default: kernels are
+  // requested by the first call that can use them (it knows the rule and the number of points)
   const char *jit_env = std::getenv("FIESTA_JIT");
   pg->jit_on = !(jit_env && jit_env[0] == '0');
   const bool jit_sync = jit_env && std::strcmp(jit_env, "sync") == 0;
+  const bool jit_eager = jit_sync || (jit_env && std::strcmp(jit_env, "eager") == 0);
   const unsigned ncpu = std::min<unsigned>(std::max(1u, std::thread::hardware_concurrency()), 32u);
   {
     std::atomic<int> next{0};
@@ -540,14 +544,14 @@ int fiesta_compile(fiesta_ctx *ctx, const fiesta_sector_desc *sectors, int32_t n
     fiesta_program_free(pg);
     return cuda_fail(ctx, e, "program upload");
   }
-  // The interpreter form is ready: the program can be integrated from here on.  The native kernels
-  // are assembled by the program's own threads from now on; the lattice rule's (the default rule)
-  // are queued at once, the other modes' when a call first asks for them.
+  // The interpreter form is ready: the program can be integrated from here on.  Native kernels are
+  // assembled by the program's own threads when a call first asks for them (or, FIESTA_JIT=eager,
+  // the lattice rule's from now on).
   pg->slots.reset(new NativeSlot[(size_t)nsectors * fx::JIT_NMODES]);
   if (pg->jit_on) {
     const unsigned nw = std::min<unsigned>(ncpu, (unsigned)nsectors);
     for (unsigned t = 0; t < nw; ++t) pg->workers.emplace_back(native_worker, pg);
-    native_request(pg, nullptr, nsectors, fx::JIT_LATTICE, false);
+    if (jit_eager) native_request(pg, nullptr, nsectors, fx::JIT_LATTICE, false);
     if (jit_sync) native_wait(pg, nullptr, nsectors, fx::JIT_LATTICE, -1.0);
   }
   *out = pg;
