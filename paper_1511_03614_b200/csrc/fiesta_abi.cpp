@@ -69,7 +69,7 @@ struct fiesta_ctx {
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   // the evaluation kernels of a pass are spread over a few side streams, so that the blocks of the
   // next sector's kernel fill the SMs while the last blocks of the previous one drain
-  static constexpr int NAUX = 4;
+  static constexpr int NAUX = 16;  // run_pass uses 4 for large kernels, more when a sector's grid is small
   cudaStream_t aux[NAUX] = {};
   cudaEvent_t aux_done[NAUX] = {};
   cudaEvent_t fork = nullptr;
