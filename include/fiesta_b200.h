@@ -176,6 +176,26 @@ int fiesta_eval_points(fiesta_ctx *ctx, const fiesta_program *prog, int32_t sect
 int fiesta_eval_points_tier(fiesta_ctx *ctx, const fiesta_program *prog, int32_t sector, int32_t tier,
                             const double *x_host, uint64_t npts, double *out_host);
 
+/* ---- mixed precision ("MPFR, Native and Mixed (default variant)") ---
+ *
+ * fiesta_set_mixed: from now on the lattice and plain-MC rules of this context evaluate every point
+ * with min_k x_k < small_x (the paper's SmallX knob) in double-double
+ * arithmetic (two doubles, ~106 bits: this library's stand-in for MPFR) and all other points in
+ * double, as before (R20).  The points, their weights and the order of the sums do not
+ * change; with no point below small_x the results are bit-identical to small_x = 0.  small_x = 0
+ * (the default) switches the mode off; small_x > 1 sends every point through the double-double
+ * walk ("-mpfr: evaluate all integration points with the use of MPFR").  Real
+ * sectors only: with the mode on, a call that selects a complex sector or uses the Vegas rule
+ * fails with FIESTA_E_RULE.  Constants enter the double-double walk as the doubles the compiler
+ * stored.  small_x < 0 or NaN: FIESTA_E_ARG. */
+int fiesta_set_mixed(fiesta_ctx *ctx, double small_x);
+
+/* Parity hook of the double-double walk: out_host[npts][K][2] = (hi, lo) with o_k(x) = hi + lo
+ * (|lo| <= ulp(hi)/2) for the real sector `sector` at x_host[npts][dim].  Complex sector:
+ * FIESTA_E_ARG. */
+int fiesta_eval_points_dd(fiesta_ctx *ctx, const fiesta_program *prog, int32_t sector, const double *x_host,
+                          uint64_t npts, double *out_host);
+
 /* The 64-bit integers t[j][k] (R2/R3) behind points j = first..first+count-1 of shift
  * (lattice) or iteration (MC/Vegas) `shift_or_iter` of the sector labelled sector_id.
  * n_lattice is used by the lattice rule only.  t_host[count][dim]. */

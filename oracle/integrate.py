@@ -120,11 +120,16 @@ def exact_sum(values):
     return ExactSum().add(values).value()
 
 
-def integrand_values(sec: SectorSpec, x, xbar=None, rdtype=LD):
+def integrand_values(sec: SectorSpec, x, xbar=None, rdtype=LD, small_x=0.0):
     """o_k at the points, shape [K, npts]; complex dtype if the sector is complex.
 
     With deformation every x becomes z(x) and the result is multiplied by det J (R11).
     The lattice / Vegas weight W is NOT included.
+
+    small_x > 0 (real sectors; the paper's "Mixed" mode, with its SmallX knob,
+    PAPER.md:447; R20): a point whose FP64 coordinates have min_k x_k < small_x takes its
+    value from the multiple-precision walk (oracle/evaluate_mp.py, FP64 constants) at that FP64
+    point, rounded to FP64.
     """
     cdtype = CLD if rdtype == LD else np.complex128
     out = []
@@ -135,6 +140,15 @@ def integrand_values(sec: SectorSpec, x, xbar=None, rdtype=LD):
             out.append(evaluate(prog, np.asarray(x, dtype=rdtype).astype(cdtype), cdtype))
         else:
             out.append(evaluate(prog, x, rdtype))
+    if small_x > 0.0:
+        if sec.is_complex or sec.deform_f_index > 0:
+            raise ValueError("the mixed mode is defined for real sectors")
+        from .evaluate_mp import evaluate_mp
+        x64 = np.asarray(x, dtype=np.float64)
+        flagged = np.nonzero(np.min(x64, axis=1) < small_x)[0]
+        for k, prog in enumerate(sec.progs):
+            for j, v in zip(flagged, evaluate_mp(prog, x64[flagged], const64=True)):
+                out[k][j] = rdtype(float(v))
     return np.stack(out)
 
 
@@ -154,14 +168,14 @@ def lattice_points(sec: SectorSpec, n_lattice, genvec, r_periodize, seed, shift_
 
 
 def lattice_partial_sums(sec: SectorSpec, n_lattice, n_shifts, genvec, r_periodize, seed, chunk=1 << 14, rdtype=LD,
-                         shifts=None, first=0, count=None):
+                         shifts=None, first=0, count=None, small_x=0.0):
     """S1[r,k,c] = sum_j g, S2[r,k,c] = sum_j g^2, SA[r,k,c] = sum_j |g|, g = W*o_k component c.
 
     Shapes [R, K, C], C = 1 (real) or 2 (Re, Im).  Each sum is the exact sum of its terms rounded
     once (O6, ExactSum); `chunk` only bounds the memory of one evaluation and cannot change a result.
     `shifts`: optional subset of shift indices to compute (the other rows stay 0); `first`, `count`:
     optional sub-range j = first..first+count-1 of the lattice; both are used to sample pieces of a
-    full-size run.
+    full-size run.  `small_x`: the mixed mode of integrand_values.
     """
     ncomp = 2 if (sec.is_complex or sec.deform_f_index > 0) else 1
     s1 = np.zeros((n_shifts, sec.K, ncomp), dtype=rdtype)
@@ -173,7 +187,7 @@ def lattice_partial_sums(sec: SectorSpec, n_lattice, n_shifts, genvec, r_periodi
         for f0 in range(first, last, chunk):
             cnt = min(chunk, last - f0)
             x, xbar, w = lattice_points(sec, n_lattice, genvec, r_periodize, seed, r, f0, cnt, rdtype)
-            vals = integrand_values(sec, x, xbar, rdtype)
+            vals = integrand_values(sec, x, xbar, rdtype, small_x)
             for k in range(sec.K):
                 for c, comp in enumerate(_components(vals[k])):
                     g = w * comp
@@ -222,7 +236,8 @@ def mc_points(sec: SectorSpec, seed, iteration, first, count, rdtype=LD):
     return t, P.unit_from_t(t, rdtype)
 
 
-def mc_partial_sums(sec: SectorSpec, npoints, seed, iteration=0, chunk=1 << 14, rdtype=LD, first=0, count=None):
+def mc_partial_sums(sec: SectorSpec, npoints, seed, iteration=0, chunk=1 << 14, rdtype=LD, first=0, count=None,
+                    small_x=0.0):
     """Plain MC (x = u, W = 1): S1[k,c] = sum_j o_k, S2[k,c] = sum_j o_k^2 over points first..first+count-1
     of the Philox MC stream (default: all npoints); exact sums rounded once (O6)."""
     ncomp = 2 if (sec.is_complex or sec.deform_f_index > 0) else 1
@@ -231,7 +246,7 @@ def mc_partial_sums(sec: SectorSpec, npoints, seed, iteration=0, chunk=1 << 14, 
     for f0 in range(first, last, chunk):
         cnt = min(chunk, last - f0)
         _, y = mc_points(sec, seed, iteration, f0, cnt, rdtype)
-        vals = integrand_values(sec, y, None, rdtype)
+        vals = integrand_values(sec, y, None, rdtype, small_x)
         for k in range(sec.K):
             for c, comp in enumerate(_components(vals[k])):
                 acc[k][c][0].add(comp)

@@ -86,6 +86,8 @@ _SIGNATURES = {
     "fiesta_select_lambda": (C.c_int, [_VP, _VP, _I32, _I32, _U64, _U64, C.c_double, _I32, _I32, C.POINTER(C.c_double),
                                        C.POINTER(_TestF)]),
     "fiesta_program_set_lambda": (C.c_int, [_VP, _VP, _I32, C.c_double]),
+    "fiesta_set_mixed": (C.c_int, [_VP, C.c_double]),
+    "fiesta_eval_points_dd": (C.c_int, [_VP, _VP, _I32, _VP, _U64, _VP]),
 }
 
 _lib = None
@@ -304,6 +306,17 @@ class Context:
                                                   _ptr(out))
         self._check(rc)
         return out[..., 0] + 1j * out[..., 1]
+
+    def set_mixed(self, small_x):
+        """Mixed precision: points with min_k x_k < small_x are evaluated in double-double (0: off)."""
+        self._check(self.lib.fiesta_set_mixed(self.handle, float(small_x)))
+
+    def eval_points_dd(self, prog, sector, x):
+        """Double-double walk of a real sector -> (hi, lo), each float64 [npts][K]."""
+        x = np.ascontiguousarray(x, dtype=np.float64)
+        out = np.zeros((x.shape[0], prog.K[int(sector)], 2))
+        self._check(self.lib.fiesta_eval_points_dd(self.handle, prog.handle, int(sector), _ptr(x), x.shape[0], _ptr(out)))
+        return out[..., 0], out[..., 1]
 
     def generate_points(self, rule, seed, sector_id, shift_or_iter, n_lattice, first, count, dim):
         t = np.zeros((count, dim), dtype=np.uint64)

@@ -81,6 +81,7 @@ struct fiesta_ctx {
   // geometry of the last single-batch pass (fiesta_chunk_sums)
   int last_nchunks = 0, last_R = 0;
   uint64_t last_chunk = 0;
+  double small_x = 0.0;  // fiesta_set_mixed
 };
 
 // One native kernel of a sector: assembled by a background thread of the program, used by
@@ -160,6 +161,8 @@ struct Plan {
   bool any_real = false, any_cplx = false;
   int Kmax = 0;
   size_t smem = 0;
+  int mem_dd = 0;             // mixed precision: spill doubles per block of the double-double walk
+  bool no_mixed = false;      // a caller that never runs phase 2 (fiesta_test_f)
 };
 
 int ilog2_exact(uint64_t n) {

@@ -126,6 +126,21 @@ static __device__ __noinline__ fx_vcoord fx_vegas_coord(uint64_t t, int nbins, c
   return fx_vegas_coord_body(t, nbins, edges);
 }
 
+// Mixed precision (R20): the points with some coordinate below small_x, as a bit mask.
+// The evaluation kernels leave them out of their sums; fx_rescue_real (fx_kernels_dd.cu) evaluates
+// exactly these in double-double.  One function, so that the two phases cannot disagree on a point.
+template <int NX, int P>
+__device__ __forceinline__ unsigned fx_flag_mask(const double (&x)[NX][P], int dim, double small_x) {
+  unsigned m = 0;
+  FX_PLOOP {
+    bool f = false;
+#pragma unroll
+    for (int k = 0; k < NX; ++k) f = f || (k < dim && x[k][p] < small_x);
+    m |= f ? 1u << p : 0u;
+  }
+  return m;
+}
+
 // Points j0..j0+P-1 of (sector, shift r / iteration) -> real x, xbar = 1-x, weight W, Vegas bins.
 // RULE is a compile-time constant: each rule has its own kernel instantiation.  INL: the per-coordinate
 // helpers inline instead of out of line -- an out-of-line call makes the kernel save the values it
@@ -201,6 +216,7 @@ __device__ __forceinline__ void fx_make_points(const fx_integrate_params &prm, i
       }
     }
   }
+  if (prm.small_x > 0.0) valid &= ~fx_flag_mask<NX, P>(x, dim, prm.small_x);  // block-uniform branch
 }
 
 // block start: shift Delta_{r,k} from the Philox shift stream (R3), Vegas grid and histogram

@@ -80,6 +80,7 @@ __device__ __forceinline__ void fxj_make_points(const fx_integrate_params &prm, 
     }
   }
   FX_PLOOP { W[p] = korobov_weight(*tf, W[p]); }
+  if (prm.small_x > 0.0) valid &= ~fx_flag_mask<NX, P>(x, dim, prm.small_x);  // mixed precision: phase 2 takes these
 }
 
 // FXJ_FMT ("%0 %1 ... %(n-1)": the marker line lists every operand once, in order) and the operand lists

@@ -70,6 +70,9 @@ struct fx_integrate_params {
   // fiesta_test_f (PAPER.md:474 -testF): one record per block, [bad points, max Im F(z), min |F(z)|^2, points]
   double *testf_out;
   double lambda_override;    // >= 0: use instead of the sector's lambda (the lambda scan); < 0: the sector's own
+  // mixed precision (fiesta_set_mixed; R20): points with some x_k < small_x are left out of the sums
+  // here and evaluated in double-double by fx_launch_rescue_real.  0: off.
+  double small_x;
 };
 
 // position in the selection of the sector a block works on
@@ -154,6 +157,10 @@ cudaError_t fx_launch_generate_points(int rule, uint64_t seed, int sector_id, in
                                       uint64_t *t_dev, cudaStream_t st);
 cudaError_t fx_launch_transform_points(int rule, const fx_transform_host &tf, const uint64_t *t_dev, uint64_t count,
                                        int dim, double *x_dev, double *xbar_dev, double *w_dev, cudaStream_t st);
+// double-double walk (fx_kernels_dd.cu): mem_doubles = 2 * n_mem_main * FX_THREADS
+cudaError_t fx_launch_eval_dd(const fx_eval_params &prm, cudaStream_t st);  // out[npts][K][hi, lo]
+cudaError_t fx_launch_rescue_real(const fx_integrate_params &prm, int nsectors, cudaStream_t st);
+size_t fx_rescue_smem_bytes(const fx_integrate_params &prm);
 cudaError_t fx_launch_fp64_peak(double *sink_dev, int iters, int blocks, cudaStream_t st);
 
 #endif

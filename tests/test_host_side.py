@@ -226,11 +226,12 @@ def test_zero_register_spills(lib):
                 name = m.group(1)
                 fallback = ("fx_integrate_cplx" in name or "fx_eval_cplx" in name or "fx_eval_real" in name or "fx_slow_" in name or
                             "fx_testf_cplx" in name or                                # the -testF diagnostic (interpreter)
+                            "fx_kernels_dd" in name or                                # the double-double rescue: rare points, C++ walk
                             re.search(r"fx_integrate_realILi\d+ELi2EE", name))        # RULE = 2: Vegas
                 (tolerated if fallback and int(m.group(2)) <= 320 and int(m.group(3)) <= 360 else bad).append(
                     (os.path.basename(path), name[:80], m.group(2), m.group(3)))
     assert not bad, bad
-    assert len(tolerated) <= 40, tolerated
+    assert len(tolerated) <= 48, tolerated
     for name, mode in (("C1", lib.RULE_LATTICE), ("C2", lib.RULE_LATTICE), ("C3", lib.RULE_LATTICE), ("C4", lib.RULE_LATTICE),
                        ("C5", lib.RULE_VEGAS), ("C3", lib.MODE_EVAL), ("C4", lib.MODE_EVAL)):
         wl = make_workload(name, nsectors=2, npoints=1 << 10)

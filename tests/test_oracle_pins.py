@@ -728,3 +728,75 @@ def test_testf_and_lambda_selection_closed_forms():
     assert float(lam) == float(max(ok, key=lambda t: t[3])[0])
     none, scan = select_lambda(cub, 1, x, lambda_max=80.0, lambda_split=2)
     assert none is None and all(t[1] > 0 for t in scan)
+
+
+# ------------------------------------------------------------------ multiple-precision walk (f1; R20)
+
+def test_mp_walk_closed_forms_under_cancellation():
+    """oracle/evaluate_mp.py against closed forms where the longdouble walk has no digit left."""
+    from fractions import Fraction
+    from oracle.evaluate_mp import evaluate_mp, to_double_double
+    # ((1+x)^3 - 1 - 3x - 3x^2) / x^3 = 1 for every x != 0
+    prog = parse(block(1, ["p[1+x[1],3]-1-3*x[1]-3*p[x[1],2]"], "f[1]/p[x[1],3]"))
+    xs = np.array([[1e-9], [2.0 ** -20], [3.7e-7], [1e-12]])
+    with mpmath.workdps(60):
+        for v in evaluate_mp(prog, xs):
+            assert abs(v - 1) < mpmath.mpf(10) ** -20          # numerator x^3 >= 1e-36, working precision 1e-60
+    ld = evaluate(prog, xs[:1], LD)
+    assert abs(float(ld[0]) - 1.0) > 1e-3                       # ... which is why the rescue exists
+    # (log(1+x) - x + x^2/2) / x^3 = sum_{k>=3} (-1)^(k+1) x^(k-3) / k, summed exactly for x = 2^-30
+    prog = parse(block(1, [], "(l[1+x[1]]-x[1]+p[x[1],2]/2)/p[x[1],3]"))
+    x = Fraction(1, 1 << 30)
+    series = sum(Fraction((-1) ** (k + 1), k) * x ** (k - 3) for k in range(3, 12))   # next term 2^-270/12
+    with mpmath.workdps(60):
+        v = evaluate_mp(prog, np.array([[float(x)]]))[0]
+        ref = mpmath.mpf(series.numerator) / mpmath.mpf(series.denominator)
+        assert abs(v - ref) < mpmath.mpf(10) ** -30             # numerator 2^-90/3 ~ 3e-28 at 1e-60: 32 digits
+    # non-integer power and the (hi, lo) split
+    prog = parse(block(2, [], "p[x[1]+x[2],-1.5]*x[1]"))
+    with mpmath.workdps(60):
+        v = evaluate_mp(prog, np.array([[0.25, 2.0]]))[0]
+        assert abs(v - mpmath.mpf("0.25") / mpmath.mpf("2.25") ** mpmath.mpf("1.5")) < mpmath.mpf(10) ** -55
+        hi, lo = to_double_double(v)
+        assert hi == float(v) and abs(mpmath.mpf(hi) + mpmath.mpf(lo) - v) < mpmath.mpf(10) ** -31 * abs(v)
+
+
+def test_mp_walk_agrees_with_longdouble_walk():
+    """Well-conditioned points of generated sectors: the two walks are the same function."""
+    from oracle.evaluate_mp import evaluate_mp
+    from workloads import make_workload
+    rng = np.random.default_rng(5)
+    for name in ("C1", "C3"):
+        wl = make_workload(name, nsectors=2, npoints=1 << 10)
+        for s in wl.sectors:
+            if s.is_complex:
+                continue
+            for text in s.texts:
+                prog = parse(text)
+                x = rng.uniform(0.05, 0.95, size=(4, prog.nvars))
+                v, mag = evaluate_with_magnitude(prog, x, LD)
+                with mpmath.workdps(60):
+                    for j, r in enumerate(evaluate_mp(prog, x)):
+                        assert abs(r - mpmath.mpf(float(v[j]))) <= 4e-16 * float(mag[j])      # float(v): one more rounding
+                    # constants as their nearest doubles (the CUDA path's immediates): first order the same
+                    for j, r in enumerate(evaluate_mp(prog, x, const64=True)):
+                        assert abs(r - mpmath.mpf(float(v[j]))) <= 8e-16 * float(mag[j])
+
+
+def test_mixed_mode_restores_closed_form():
+    """integrand_values(small_x=...): int_0^1 int_0^1 ((1+x)^3-1-3x-3x^2)/x^3 (1+y) dx dy = 3/2.  The lattice rule's
+    periodising transform puts points at x ~ 1e-12, where the numerator is rounding noise over x^3."""
+    text = block(2, ["p[1+x[1],3]-1-3*x[1]-3*p[x[1],2]"], "f[1]/p[x[1],3]*(1+x[2])")
+    sec = SectorSpec([text])
+    nl = 1 << 10
+    gv = P.korobov_genvec(korobov_a(nl, 2), nl, 2)
+    s1, s2, _ = lattice_partial_sums(sec, nl, 4, gv, 3, 7, small_x=0.02)
+    val, err = estimate_from_sums(s1, s2, nl)
+    assert abs(float(val[0, 0]) - 1.5) < 1e-9 and float(err[0, 0]) < 1e-8
+    s1, s2, _ = lattice_partial_sums(sec, nl, 4, gv, 3, 7)          # long double everywhere: lost
+    val, err = estimate_from_sums(s1, s2, nl)
+    assert abs(float(val[0, 0]) - 1.5) > 1.0
+    # small_x below every coordinate: nothing is flagged, nothing changes
+    a = mc_partial_sums(sec, 1 << 8, 3)
+    b = mc_partial_sums(sec, 1 << 8, 3, small_x=1e-300)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
