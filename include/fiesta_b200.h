@@ -186,7 +186,8 @@ int fiesta_eval_points_tier(fiesta_ctx *ctx, const fiesta_program *prog, int32_t
  * (the default) switches the mode off; small_x > 1 sends every point through the double-double
  * walk ("-mpfr: evaluate all integration points with the use of MPFR").  Real
  * sectors only: with the mode on, a call that selects a complex sector or uses the Vegas rule
- * fails with FIESTA_E_RULE.  Constants enter the double-double walk as the doubles the compiler
+ * fails with FIESTA_E_RULE, and so does FIESTA_TIER_NATIVE (the first phase runs on the interpreter
+ * kernels; the default tier choice follows).  Constants enter the double-double walk as the doubles the compiler
  * stored.  small_x < 0 or NaN: FIESTA_E_ARG. */
 int fiesta_set_mixed(fiesta_ctx *ctx, double small_x);
 

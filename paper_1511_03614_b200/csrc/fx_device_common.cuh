@@ -216,7 +216,9 @@ __device__ __forceinline__ void fx_make_points(const fx_integrate_params &prm, i
       }
     }
   }
+#ifndef FX_NO_MIXED_MASK  // the native templates and the complex kernels never run with the mixed mode on
   if (prm.small_x > 0.0) valid &= ~fx_flag_mask<NX, P>(x, dim, prm.small_x);  // block-uniform branch
+#endif
 }
 
 // block start: shift Delta_{r,k} from the Philox shift stream (R3), Vegas grid and histogram

@@ -19,6 +19,7 @@
 //   integrate: [h2[0..P) if Vegas] valid acc W[0..P) x[0][0..P) x[1][..) ...
 //   eval:      valid out x[0][0..P) ...
 #define FX_WANT(is_cplx, nx, p) 0  // no interpreter fast path in this translation unit
+#define FX_NO_MIXED_MASK  // fiesta_set_mixed: phase 1 runs on the real interpreter kernels only
 #include "fx_device_common.cuh"
 
 #ifndef FXJ_NX
@@ -45,7 +46,8 @@ static __device__ __noinline__ fxj_xs fxj_transform_any(const fx_transform *tf, 
 
 // Lattice points of one pass, inline (2 points x NX coordinates; with 4 points live inlining was slower) and
 // without xbar = 1-x, which real programs never read.  Same arithmetic and order as
-// fx_make_points<FIESTA_RULE_LATTICE>: x and W are bit-identical.  (The per-point branch on the weight
+// fx_make_points<FIESTA_RULE_LATTICE>: x and W are bit-identical -- except that it knows nothing of the mixed
+// mode's mask (fx_flag_mask): with fiesta_set_mixed on, phase 1 runs on the interpreter kernels.  (The per-point branch on the weight
 // also keeps ptxas from interleaving all 2 NX transforms at once, which costs it spills.)
 template <int NX, int P>
 __device__ __forceinline__ void fxj_make_points(const fx_integrate_params &prm, int dim, const uint64_t *sh_delta,
@@ -80,7 +82,6 @@ __device__ __forceinline__ void fxj_make_points(const fx_integrate_params &prm, 
     }
   }
   FX_PLOOP { W[p] = korobov_weight(*tf, W[p]); }
-  if (prm.small_x > 0.0) valid &= ~fx_flag_mask<NX, P>(x, dim, prm.small_x);  // mixed precision: phase 2 takes these
 }
 
 // FXJ_FMT ("%0 %1 ... %(n-1)": the marker line lists every operand once, in order) and the operand lists

@@ -18,6 +18,7 @@
 // build.py passes the operand lists as macros: FXJ_DFMT / FXJ_FMT ("%0 %1 ..."), FXJ_GH_OUTS
 // ("=d"(gh[0]), ...), FXJ_X_INS ("d"(xv[0]), ...), FXJ_Z_INS ("d"(xv[0]), "d"(zi[0]), ...).
 #define FX_WANT(is_cplx, nx, p) 0  // no interpreter fast path in this translation unit
+#define FX_NO_MIXED_MASK  // fiesta_set_mixed: phase 1 runs on the real interpreter kernels only
 #include "fx_device_common.cuh"
 #include "fx_deform.cuh"
 

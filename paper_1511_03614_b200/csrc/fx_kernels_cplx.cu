@@ -10,6 +10,7 @@
 #error "compile with -DFX_N=<dimension 1..8>"
 #endif
 #define FX_WANT(is_cplx, nx, p) ((nx) == FX_N && (p) == 1)  // real (deformation program) and complex, P = 2
+#define FX_NO_MIXED_MASK  // fiesta_set_mixed: phase 1 runs on the real interpreter kernels only
 #include "fx_device_common.cuh"
 #include "fx_deform.cuh"
 
