@@ -272,6 +272,12 @@ class Timer:
         return step_ms, kern_ms, launches, tiers
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of one native-kernel launch, from the committed ncu --set full
+# captures (profiles/r02_ncu_fxj_integrate_c3.md, _c4.md, _c5.md): the points are made on the device and a block
+# writes one 256-byte record, so the traffic of the ALU-bound kernels is the program text and the parameters
+NCU_DRAM_BYTES = {"C3": 56832, "C4": 54784, "C5": 38656}
+
+
 def roofline_of(wl, prog, S, kern_ms, peak_live, tiers):
     """bound 'alu': algorithmic FP64 flops of one pass / the evaluation kernels' time (CUDA events inside the
     library, fiesta_last_timing) against the FP64 peak derived in DESIGN.md section 6."""
@@ -284,7 +290,7 @@ def roofline_of(wl, prog, S, kern_ms, peak_live, tiers):
     ach_prog = prog_flops * pts / (kms * 1e-3) / 1e12
     native = tiers[1] == 0
     return {"bound": "alu", "achieved": ach, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach / FP64_PEAK_TFLOPS,
-            "traffic": None,
+            "traffic": NCU_DRAM_BYTES.get(wl.name) if native else None, "traffic_unit": "bytes per launch (dram read + write)",
             "achieved_program_only": ach_prog, "frac_program_only": ach_prog / FP64_PEAK_TFLOPS,
             "flops_per_point": prog_flops + over, "flops_per_point_program": prog_flops,
             "flops_per_point_path_overhead": over,
