@@ -12,5 +12,6 @@ from .binding import (  # noqa: F401
 )
 
 from .pool import IntegrationPool, ResultStore  # noqa: F401,E402
+from .bisection import bisect_sector, bisect_text  # noqa: F401,E402
 
 load = load_library

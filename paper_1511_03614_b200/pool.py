@@ -21,7 +21,17 @@ method, only which sectors go where and when:
     flushed to disk; a record carries the signature of what produced it (rule, points, seed, the
     sector's texts), so a later run skips exactly the work that is already there;
   * totals: when every sector of the part is there, the ranks exchange their records once
-    (sharding.gather_results) and fiesta_combine sums per order.
+    (sharding.gather_results) and fiesta_combine sums per order;
+  * frozen workers: "if some of the slave jobs become frozen during the integration, FIESTA is
+    capable of resubmitting their tasks to other nodes"; jobs whose integrators "are initialized
+    improperly" are passed over.  Here every rank can read every rank's store file
+    (a shared file system): a rank that still owes sectors and whose file has not grown for
+    `stale_after` seconds -- or was never created -- counts as frozen (frozen_ranks), and a rank
+    that is through with its own share takes those sectors over (adopt), cheapest first, i.e. from
+    the far end of the owner's queue.  A sector's result does not depend on who computes it (same
+    sector id, seed and rule: the same bits), so a slow owner that finishes after all merely writes
+    a duplicate record.  With a dead rank a collective would hang: results(collective=False) reads
+    the part's records from the store files instead.
 """
 from __future__ import annotations
 
@@ -29,6 +39,7 @@ import ctypes as C
 import hashlib
 import json
 import os
+import time
 
 import numpy as np
 
@@ -62,6 +73,23 @@ class ResultStore:
             for name in sorted(os.listdir(d)):      # every rank's file: a restart may use another number of ranks
                 if name.startswith(base + ".rank"):
                     self._load(os.path.join(d, name))
+
+    def refresh(self):
+        """Read every rank's file again: what the other ranks have stored since this object was made."""
+        if self.path is None:
+            return
+        d = os.path.dirname(os.path.abspath(self.path))
+        base = os.path.basename(self.path)
+        for name in sorted(os.listdir(d)):
+            if name.startswith(base + ".rank"):
+                self._load(os.path.join(d, name))
+
+    def age(self, rank, now=None):
+        """Seconds since rank's file was last written; None if it does not exist."""
+        f = f"{self.path}.rank{rank}"
+        if self.path is None or not os.path.exists(f):
+            return None
+        return (time.time() if now is None else now) - os.path.getmtime(f)
 
     def _load(self, file):
         with open(file) as fh:
@@ -151,7 +179,10 @@ class IntegrationPool:
             costs = [sum(len(t) for t in s.texts) * float(npoints) for s in sectors]
         self.costs = [float(costs[i]) for i in self.indices]
         shares = partition_sectors(self.costs, self.world)
-        self.my_local = sorted(shares[self.rank], key=lambda j: (-self.costs[j], j))   # largest first
+        self.shares = [sorted(sh, key=lambda j: (-self.costs[j], j)) for sh in shares]  # every rank's queue, largest first
+        self.my_local = self.shares[self.rank]
+        self.started = time.time()
+        self.n_adopted = 0                                  # sectors taken over from frozen ranks
         self.sigs = {j: _signature(sectors[self.indices[j]], dim, rule, npoints, seed) for j in range(len(self.indices))}
         self.store = ResultStore(store_path, self.rank)
         self.n_integrated = 0                               # sectors this object sent to the GPU
@@ -165,6 +196,55 @@ class IntegrationPool:
         """Work the queue off (at most max_groups groups: a time limit).  Returns True when this rank is done."""
         todo = self.pending()
         self.n_from_store = len(self.my_local) - len(todo)
+        self._work(todo, max_groups)
+        return not self.pending()
+
+    def frozen_ranks(self, stale_after):
+        """Other ranks that still owe sectors and whose store file has not been written for `stale_after`
+        seconds -- or does not exist `stale_after` seconds after this pool was made (a worker that never
+        came up).  Reads the store files again first."""
+        if self.store.path is None:
+            raise RuntimeError("frozen workers are recognised by their store files: the pool needs a store_path")
+        self.store.refresh()
+        now = time.time()
+        out = []
+        for r in range(self.world):
+            if r == self.rank or all(self.store.get(self.sigs[j], self.K) is not None for j in self.shares[r]):
+                continue
+            age = self.store.age(r, now)
+            if (now - self.started if age is None else age) >= stale_after:
+                out.append(r)
+        return out
+
+    def adopt(self, ranks, max_groups=None):
+        """Integrate what the given (frozen) ranks still owe, cheapest sectors first -- the far end of their
+        queues, which a merely slow owner reaches last.  Returns the number of sectors taken over."""
+        self.store.refresh()
+        todo = [j for r in ranks for j in self.shares[r] if self.store.get(self.sigs[j], self.K) is None]
+        todo.sort(key=lambda j: (self.costs[j], j))
+        before = self.n_integrated
+        self._work(todo, max_groups)
+        self.n_adopted += self.n_integrated - before
+        return self.n_integrated - before
+
+    def run_to_completion(self, stale_after, poll=1.0, timeout=None):
+        """run(), then watch the other ranks: adopt the sectors of those that freeze, until the whole part is in
+        the store (True) or `timeout` seconds have passed (False)."""
+        self.run()
+        t0 = time.time()
+        while True:
+            self.store.refresh()
+            if all(self.store.get(self.sigs[j], self.K) is not None for j in range(len(self.indices))):
+                return True
+            frozen = self.frozen_ranks(stale_after)
+            if frozen:
+                self.adopt(frozen)
+                continue
+            if timeout is not None and time.time() - t0 > timeout:
+                return False
+            time.sleep(poll)
+
+    def _work(self, todo, max_groups=None):
         groups = [todo[i:i + self.group] for i in range(0, len(todo), self.group)]
         if max_groups is not None:
             groups = groups[:max_groups]
@@ -184,10 +264,19 @@ class IntegrationPool:
             close = getattr(progs.pop(g), "close", None)
             if close:
                 close()
-        return not self.pending()
 
-    def results(self):
-        """[sectors of the part][K] of ALL ranks (one gather); raises if some sector is not there yet."""
+    def results(self, collective=True):
+        """[sectors of the part][K] of ALL ranks; raises if some sector is not there yet.  collective=True: one
+        gather of every rank's own share; False: from the store files alone (no rank waits for another)."""
+        if not collective:
+            self.store.refresh()
+            out = np.zeros((len(self.indices), self.K), dtype=RESULT_DTYPE)
+            for j in range(len(self.indices)):
+                row = self.store.get(self.sigs[j], self.K)
+                if row is None:
+                    raise RuntimeError(f"sector {self.sectors[self.indices[j]].sector_id} has not been integrated yet")
+                out[j] = row
+            return out
         mine = self.my_local
         local = np.zeros((len(mine), self.K), dtype=RESULT_DTYPE)
         for a, j in enumerate(mine):
@@ -197,6 +286,6 @@ class IntegrationPool:
             local[a] = row
         return gather_results(local, mine, len(self.indices), self.dist, self.device)
 
-    def totals(self):
+    def totals(self, collective=True):
         """Per order: sum over the part's sectors, errors in mean square."""
-        return combine(self.results())
+        return combine(self.results(collective))

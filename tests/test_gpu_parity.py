@@ -469,6 +469,42 @@ def test_lambda_zero_reproduces_real_path(fb, ctx):
     assert np.allclose(b.real[ok], a.real[ok], rtol=1e-11) and np.all(np.abs(b.imag[ok]) <= 1e-11 * np.abs(a.real[ok]))
 
 
+def test_bisected_cube_parts_add_up(fb, ctx):
+    """PAPER.md:406 BisectionVariables (bisection.py): the parts of a bisected integrand are ordinary sectors --
+    per-point parity with the oracle on the rewritten texts -- and their integrals add up: to the closed forms
+    of the 1-D contour integrals (the zero of F at 0.3 lies in the lower part), and to the unbisected integral
+    of a generated real sector."""
+    from conftest import golden
+    from paper_1511_03614_b200.bisection import bisect_sector
+    g = golden("contour_1d_closed_forms.txt")
+    texts = [block(1, ["x[1]-0.3"], f) for f in ("1/f[1]", "l[f[1]]", "p[f[1],-0.5]")]
+    sec = one_sector(texts, is_complex=True, deform_f_index=1, lam=0.5, sector_id=3)
+    parts = bisect_sector(sec, [1], points=0.5)
+    prog = ctx.compile(parts, 1)
+    x = np.random.default_rng(4).random((300, 1))
+    for si, part in enumerate(parts):
+        ref, mag = oracle_values_and_magnitude(spec(part), x)
+        assert check_points(ctx.eval_points(prog, si, x), ref, mag) <= 1.0
+    res = ctx.integrate(prog, 8 << 13, fb.Rule(kind=fb.RULE_LATTICE, n_shifts=8, korobov_a=1, periodize_r=3), 5)
+    for k, key in enumerate(("inv", "log", "rsqrt")):
+        re, im = float(g[key + "_re"]), float(g[key + "_im"])
+        got_re, got_im = res[0][k]["re"] + res[1][k]["re"], res[0][k]["im"] + res[1][k]["im"]
+        assert abs(got_re - re) < 1e-8 and abs(got_im - im) < 1e-8
+    prog.close()
+    wl = make_workload("C2", nsectors=1, npoints=1 << 16, n_shifts=8)
+    parts = bisect_sector(wl.sectors[0], [1, 4], points=[0.5, 0.25])
+    rule = fb.Rule.from_workload(wl)
+    whole_prog, parts_prog = ctx.compile(wl.sectors, wl.dim), ctx.compile(parts, wl.dim)
+    whole = ctx.integrate(whole_prog, wl.npoints, rule, wl.seed)[0]
+    res = ctx.integrate(parts_prog, wl.npoints, rule, wl.seed)
+    for k in range(len(whole)):
+        total = sum(res[h][k]["re"] for h in range(4))
+        sigma = np.sqrt(whole[k]["re_err"] ** 2 + sum(res[h][k]["re_err"] ** 2 for h in range(4)))
+        assert abs(total - whole[k]["re"]) <= 5 * sigma + 1e-12 * abs(whole[k]["re"])
+    whole_prog.close()
+    parts_prog.close()
+
+
 # ------------------------------------------------------------------------------ -testF, choice of lambda
 
 def test_testf_and_lambda_scan(fb, ctx):

@@ -155,3 +155,111 @@ def test_pool_world_size_2_gloo(tmp_path):
     pool = IntegrationPool(ctx, ns["sectors"](17), 1, ns["Rule"](kind=1), 1000, 3, store_path=str(tmp_path / "db"), group=4,
                            costs=[(i * 5) % 7 + 1 for i in range(17)])
     assert pool.run() and ctx.integrated == []
+
+
+# ------------------------------------------------------------------ bisection of the cube
+
+def test_bisection_rewrites_the_text_correctly():
+    """bisect_sector against the change of variables it stands for, through the ORACLE's parser and walker:
+    part(t) = jacobian * f(x(t)), x_k = p t (lower) or 1 - (1-p) t (upper); the parts cover the cube once."""
+    import numpy as np
+    from oracle.evaluate import LD, evaluate, evaluate_with_magnitude
+    from oracle.parser import parse
+    from paper_1511_03614_b200.bisection import bisect_sector, bisect_text
+    from workloads import SectorText, make_workload
+    wl = make_workload("C2", nsectors=1, npoints=1 << 10)
+    s = wl.sectors[0]
+    parts = bisect_sector(s, [2, 5], points=[0.5, 0.25])    # dyadic: 1 - p is exact in the text as well
+    assert [p.sector_id for p in parts] == [4 * s.sector_id + h for h in range(4)]
+    assert parts[1].meta["halves"] == {2: "upper", 5: "lower"} and parts[2].meta["halves"] == {2: "lower", 5: "upper"}
+    rng = np.random.default_rng(0)
+    t = rng.random((50, wl.dim)).astype(LD)
+    for h, part in enumerate(parts):
+        x = t.copy()
+        jac = LD(1)
+        for bit, (k, p) in enumerate(((2, LD(0.5)), (5, LD(0.25)))):
+            if (h >> bit) & 1:
+                x[:, k - 1] = 1 - (1 - p) * t[:, k - 1]
+                jac = jac * (1 - p)
+            else:
+                x[:, k - 1] = p * t[:, k - 1]
+                jac = jac * p
+        for text, ptext in zip(s.texts, part.texts):
+            ref, mag = evaluate_with_magnitude(parse(text), x)
+            got = evaluate(parse(ptext), t)
+            assert np.all(np.abs(got - jac * ref) <= 1e-17 * jac * mag)
+    # a 1-D integrand integrated exactly: x^3 over [0,1] = 1/4 from the two parts' antiderivatives
+    lo, up = (parse(bisect_text("1;\n0;\np[x[1],3];\n|", {1: (0.25, u)})) for u in (False, True))
+    nodes, weights = np.polynomial.legendre.leggauss(4)
+    tt = ((nodes + 1) / 2)[:, None].astype(LD)
+    total = sum(float(np.sum(weights / 2 * evaluate(prog, tt).astype(float))) for prog in (lo, up))
+    assert abs(total - 0.25) < 1e-15
+    # errors
+    import pytest
+    with pytest.raises(ValueError):
+        bisect_sector(s, [2, 2])
+    with pytest.raises(ValueError):
+        bisect_sector(s, [wl.dim + 1])
+    with pytest.raises(ValueError):
+        bisect_sector(s, [1], points=1.0)
+    tiny = bisect_sector(SectorText(sector_id=0, texts=["1;\n0;\nx[1];\n|"]), [1], points=1e-7)   # exponent literals parse
+    assert abs(float(evaluate(parse(tiny[0].texts[0]), np.array([[0.5]], dtype=LD))[0]) - 0.5e-14) < 1e-28
+
+
+class _StubDist:
+    """torch.distributed's query functions for a rank that never talks to anybody (the frozen-worker tests)."""
+
+    def __init__(self, rank, world):
+        self.rank, self.world = rank, world
+
+    def is_initialized(self):
+        return True
+
+    def get_rank(self):
+        return self.rank
+
+    def get_world_size(self):
+        return self.world
+
+
+def test_pool_resubmits_the_work_of_frozen_ranks(tmp_path, lib):
+    """a rank that froze mid-way and one that never came up; the surviving rank takes their sectors
+    over through the store files, and the totals are those of an undisturbed job."""
+    import time
+    from paper_1511_03614_b200.pool import IntegrationPool
+    ns = _ns()
+    secs, rule = ns["sectors"](20), ns["Rule"](kind=1)
+    costs = [(i * 3) % 7 + 1 for i in range(20)]
+    path = str(tmp_path / "db")
+    mk = lambda r, ctx: IntegrationPool(ctx, secs, 1, rule, 1000, 9, store_path=path, group=2, costs=costs, dist=_StubDist(r, 3))
+    ctx1 = ns["FakeCtx"]()
+    p1 = mk(1, ctx1)
+    assert not p1.run(max_groups=1)                       # rank 1 stores one group, then hangs; rank 2 never starts
+    ctx0 = ns["FakeCtx"]()
+    p0 = mk(0, ctx0)
+    assert p0.run() and p0.frozen_ranks(stale_after=3600.0) == []      # nobody is late yet
+    with pytest.raises(RuntimeError):
+        p0.results(collective=False)
+    time.sleep(0.05)
+    assert p0.frozen_ranks(stale_after=0.01) == [1, 2]
+    done1 = {s for g in ctx1.integrated for s in g}
+    n = p0.adopt([1, 2])
+    owed = set(100 + j for r in (1, 2) for j in p0.shares[r]) - done1
+    adopted = [s for g in ctx0.integrated for s in g][len(p0.my_local):]
+    assert n == len(owed) == p0.n_adopted and set(adopted) == owed
+    assert [costs[s - 100] for s in adopted] == sorted(costs[s - 100] for s in adopted)    # cheapest first
+    res = p0.results(collective=False)
+    assert all(res[i, 0]["re"] == 100 + i for i in range(20))
+    assert p0.totals(collective=False)[0]["re"] == sum(100 + i for i in range(20))
+    assert p0.frozen_ranks(stale_after=0.0) == []         # nothing is owed any more
+    # the slow rank wakes up: everything it owed is in the store, it computes nothing and sees the same totals
+    ctx1b = ns["FakeCtx"]()
+    p1b = mk(1, ctx1b)
+    assert p1b.run() and ctx1b.integrated == []
+    assert p1b.totals(collective=False).tobytes() == p0.totals(collective=False).tobytes()
+    # run_to_completion: own share, then the frozen ranks' (a fresh store)
+    path2 = str(tmp_path / "db2")
+    ctx = ns["FakeCtx"]()
+    p = IntegrationPool(ctx, secs, 1, rule, 1000, 9, store_path=path2, group=4, costs=costs, dist=_StubDist(2, 3))
+    assert p.run_to_completion(stale_after=0.0, poll=0.01, timeout=5.0)
+    assert sorted(s for g in ctx.integrated for s in g) == [100 + i for i in range(20)] and p.n_adopted == 20 - len(p.my_local)
