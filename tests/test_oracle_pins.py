@@ -800,3 +800,77 @@ def test_mixed_mode_restores_closed_form():
     a = mc_partial_sums(sec, 1 << 8, 3)
     b = mc_partial_sums(sec, 1 << 8, 3, small_x=1e-300)
     assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+
+
+# ------------------------------------------------------------------ deterministic cubature (f4; R21)
+
+def test_genz_malik_rule_degrees_of_exactness():
+    """oracle/cubature.py: the degree-7 rule integrates every monomial of total degree <= 7 exactly over an
+    arbitrary box, the embedded rule those of degree <= 5 -- which fixes every weight and node radius -- and
+    neither goes one degree further."""
+    from fractions import Fraction
+    from oracle.cubature import genz_malik, rule_on_box
+    rng = np.random.default_rng(12)
+    for n in (2, 3, 5):
+        off, w7, w5 = genz_malik(n)
+        assert off.shape[0] == 1 + 4 * n + 2 * n * (n - 1) + 2 ** n
+        assert abs(float(np.sum(w7)) - 1) < 1e-17 and abs(float(np.sum(w5)) - 1) < 1e-17
+        c = np.array([Fraction(int(v), 64) for v in rng.integers(20, 44, size=n)])
+        h = np.array([Fraction(int(v), 64) for v in rng.integers(2, 20, size=n)])
+
+        def exact(a):       # prod_k int_{c-h}^{c+h} x^a dx
+            out = Fraction(1)
+            for k in range(n):
+                out *= ((c[k] + h[k]) ** (a[k] + 1) - (c[k] - h[k]) ** (a[k] + 1)) / (a[k] + 1)
+            return float(out)
+
+        cf, hf = np.array([float(v) for v in c]), np.array([float(v) for v in h])
+        worst7 = worst5 = 0.0
+        for a in itertools.product(range(9), repeat=n):
+            deg = sum(a)
+            if deg > 8 or (n == 5 and deg > 6 and max(a) < 3 and rng.random() < 0.8):
+                continue
+            f = lambda x, a=a: np.prod(x ** np.array(a), axis=1)[None, :]
+            i7, i5, _ = rule_on_box(f, cf, hf, (off, w7, w5))
+            ex = exact(a)
+            r7, r5 = abs(float(i7[0]) - ex) / ex, abs(float(i5[0]) - ex) / ex
+            if deg <= 7:
+                assert r7 < 1e-16, (n, a, r7)
+            if deg <= 5:
+                assert r5 < 1e-16, (n, a, r5)
+            if deg == 8 and max(a) == 8:
+                worst7 = max(worst7, r7)
+            if deg == 6 and max(a) == 6:
+                worst5 = max(worst5, r5)
+        assert worst7 > 1e-8 and worst5 > 1e-8
+
+
+def test_cubature_rounds_closed_forms_and_bookkeeping():
+    from oracle.cubature import integrate_cubature, rule_on_box, sector_components
+    # int_0^1 int_0^1 (1+x+y)^-2 = ln(4/3); a sector text through the oracle's evaluator
+    sec = SectorSpec([block(2, ["1+x[1]+x[2]"], "p[f[1],-2]"), block(2, ["1+x[1]+x[2]"], "l[f[1]]")])
+    f = sector_components(sec)
+    total, err, neval, boxes = integrate_cubature(f, 2, epsrel=1e-10, maxeval=1 << 16, return_boxes=True)
+    exact0 = math.log(4.0 / 3.0)
+    exact1 = float(mpmath.quad(lambda x, y: mpmath.log(1 + x + y), [0, 1], [0, 1]))
+    assert abs(float(total[0]) - exact0) <= float(err[0]) <= 1e-10 * exact0
+    assert abs(float(total[1]) - exact1) <= float(err[1]) <= 1e-10 * exact1
+    assert neval == 17 * (2 * len(boxes) - 1)                       # every split adds two boxes' worth and removes one box
+    assert abs(sum(float(np.prod(2 * b["h"])) for b in boxes) - 1) < 1e-15          # the boxes tile the cube
+    # maxeval is respected and reported honestly
+    total2, err2, neval2, nb2 = integrate_cubature(f, 2, epsrel=1e-14, maxeval=2000)
+    assert neval2 <= 2000 and float(err2[0]) > 1e-14 * exact0 and abs(float(total2[0]) - exact0) <= float(err2[0])
+    # the split axis follows the fourth difference: a function of x2 alone is never cut along x1
+    g = lambda x: (1 / (LD(0.05) + x[:, 1] ** 2))[None, :]
+    _, _, d = rule_on_box(g, [0.5, 0.5], [0.5, 0.5])
+    assert d[0] < 1e-16 * d[1] and d[1] > 0
+    _, _, _, bx = integrate_cubature(g, 2, epsrel=1e-8, maxeval=1 << 15, return_boxes=True)
+    assert len(bx) > 8 and all(float(b["h"][0]) == 0.5 for b in bx)
+    # a peaked integrand: the boxes crowd around the peak (adaptivity), and the result is right
+    peak = lambda x: (1 / (LD(1e-2) + (x[:, 0] - LD(0.3)) ** 2 + (x[:, 1] - LD(0.7)) ** 2))[None, :]
+    tot, er, _, bx = integrate_cubature(peak, 2, epsrel=1e-7, maxeval=1 << 18, return_boxes=True)
+    ref = float(mpmath.quad(lambda x, y: 1 / (mpmath.mpf("0.01") + (x - 0.3) ** 2 + (y - 0.7) ** 2), [0, 0.3, 1], [0, 0.7, 1]))
+    assert abs(float(tot[0]) - ref) <= 10 * float(er[0]) and float(er[0]) <= 1e-7 * ref
+    small = min(float(np.prod(2 * b["h"])) for b in bx)
+    where = [b for b in bx if float(np.prod(2 * b["h"])) == small]
+    assert all(abs(float(b["c"][0]) - 0.3) < 0.2 and abs(float(b["c"][1]) - 0.7) < 0.2 for b in where)
