@@ -176,6 +176,31 @@ int fiesta_eval_points(fiesta_ctx *ctx, const fiesta_program *prog, int32_t sect
 int fiesta_eval_points_tier(fiesta_ctx *ctx, const fiesta_program *prog, int32_t sector, int32_t tier,
                             const double *x_host, uint64_t npts, double *out_host);
 
+/* ---- deterministic integrator (PAPER.md:412 `CurrentIntegrator -> cuhreCuba`) ------
+ *
+ * A Cuhre-like globally adaptive cubature on the same evaluator (R21): the degree-7 rule of
+ * Genz and Malik with its embedded degree-5 rule on boxes of the unit cube (1 + 4n + 2n(n-1) + 2^n
+ * nodes per box; the error of a box is |I7 - I5| per component).  Rounds: the boxes that carry the
+ * worst half of the summed error are halved along the axis of their largest fourth difference, until
+ * for every order and component  sum err <= max(epsabs, epsrel |sum I7|)  or another round would pass
+ * maxeval integrand evaluations.  No random numbers: a call is reproducible bit by bit.
+ *
+ * sectors[nsel] (NULL: 0..nsel-1), all with the same number of orders K; dim >= 2 (FIESTA_E_DIM);
+ * tier as for fiesta_eval_points_tier.  out[nsel][K]: re / im = the estimates, re_err / im_err = the
+ * summed box errors, chi2 = 0, neval = integrand evaluations spent on the sector; nboxes_out[nsel]
+ * (may be NULL): boxes at the end.  A NaN or Inf at a node ends the sector's rounds; the call then
+ * returns FIESTA_E_NONFINITE after filling out (n_nonfinite > 0). */
+int fiesta_integrate_cubature(fiesta_ctx *ctx, const fiesta_program *prog, const int32_t *sectors, int32_t nsel,
+                              double epsrel, double epsabs, uint64_t maxeval, int32_t tier, fiesta_result *out,
+                              uint64_t *nboxes_out);
+
+/* Parity hook: the rule on caller-given boxes.  boxes_host[nboxes][2][dim] = centre, half-widths (inside
+ * the unit cube, else FIESTA_E_ARG); i7_host, i5_host [nboxes][K][2] (re, im), fourth_host[nboxes][dim]
+ * (fourth differences summed over the components), axis_host[nboxes]; any output may be NULL. */
+int fiesta_cubature_rule(fiesta_ctx *ctx, const fiesta_program *prog, int32_t sector, int32_t tier,
+                         const double *boxes_host, uint64_t nboxes, double *i7_host, double *i5_host,
+                         double *fourth_host, int32_t *axis_host);
+
 /* ---- mixed precision ("MPFR, Native and Mixed (default variant)") ---
  *
  * fiesta_set_mixed: from now on the lattice and plain-MC rules of this context evaluate every point

@@ -27,6 +27,10 @@ Pin status (see tests/test_oracle_*.py, all `-m "not gpu"`):
                             lambda-independence (Cauchy)
   det J                     pinned: cofactor expansion, numpy.linalg.det
   Vegas refine / combine    pinned: invariants, closed forms, 4-sigma coverage
+  multiple-precision walk   pinned: closed forms under cancellation, agreement with
+  (evaluate_mp, mixed sums)  the long-double walk, 3/2 restored by small_x (R20)
+  cubature (R21)            pinned: degrees of exactness 7 / 5 on every monomial,
+                            closed forms, tiling, evaluation count, split axis
   the five BASELINE configs parity unpinned against external truth (random
                             polynomials have no closed form); covered by the
                             component pins above.

@@ -86,6 +86,8 @@ _SIGNATURES = {
     "fiesta_select_lambda": (C.c_int, [_VP, _VP, _I32, _I32, _U64, _U64, C.c_double, _I32, _I32, C.POINTER(C.c_double),
                                        C.POINTER(_TestF)]),
     "fiesta_program_set_lambda": (C.c_int, [_VP, _VP, _I32, C.c_double]),
+    "fiesta_integrate_cubature": (C.c_int, [_VP, _VP, _VP, _I32, C.c_double, C.c_double, _U64, _I32, _VP, _VP]),
+    "fiesta_cubature_rule": (C.c_int, [_VP, _VP, _I32, _I32, _VP, _U64, _VP, _VP, _VP, _VP]),
     "fiesta_set_mixed": (C.c_int, [_VP, C.c_double]),
     "fiesta_eval_points_dd": (C.c_int, [_VP, _VP, _I32, _VP, _U64, _VP]),
 }
@@ -306,6 +308,26 @@ class Context:
                                                   _ptr(out))
         self._check(rc)
         return out[..., 0] + 1j * out[..., 1]
+
+    def integrate_cubature(self, prog, epsrel=1e-6, epsabs=0.0, maxeval=1 << 22, sectors=None, tier=TIER_ANY,
+                           allow_nonfinite=False):
+        """Deterministic adaptive cubature -> (record array [nsectors][K] of RESULT_DTYPE, boxes per sector)."""
+        sel, nsel, idx = self._sel(prog, sectors)
+        out = np.zeros((nsel, prog.K[idx[0]]), dtype=RESULT_DTYPE)
+        nboxes = np.zeros(nsel, dtype=np.uint64)
+        self._check(self.lib.fiesta_integrate_cubature(self.handle, prog.handle, _ptr(sel), nsel, float(epsrel), float(epsabs),
+                                                       int(maxeval), int(tier), _ptr(out), _ptr(nboxes)), allow_nonfinite)
+        return out, nboxes
+
+    def cubature_rule(self, prog, sector, boxes, tier=TIER_ANY):
+        """boxes [nb][2][dim] (centre, half-widths) -> I7, I5 complex [nb][K], fourth differences [nb][dim], axis [nb]."""
+        boxes = np.ascontiguousarray(boxes, dtype=np.float64).reshape(-1, 2, prog.dim)
+        nb, K = boxes.shape[0], prog.K[int(sector)]
+        i7, i5 = np.zeros((nb, K, 2)), np.zeros((nb, K, 2))
+        fourth, axis = np.zeros((nb, prog.dim)), np.zeros(nb, dtype=np.int32)
+        self._check(self.lib.fiesta_cubature_rule(self.handle, prog.handle, int(sector), int(tier), _ptr(boxes), nb, _ptr(i7),
+                                                  _ptr(i5), _ptr(fourth), _ptr(axis)))
+        return i7[..., 0] + 1j * i7[..., 1], i5[..., 0] + 1j * i5[..., 1], fourth, axis
 
     def set_mixed(self, small_x):
         """Mixed precision: points with min_k x_k < small_x are evaluated in double-double (0: off)."""

@@ -122,6 +122,7 @@ def build(force=False, verbose=False):
     cu("fx_kernels_real", "fx_kernels_real.cu")
     cu("fx_kernels_small", "fx_kernels_small.cu")
     cu("fx_kernels_dd", "fx_kernels_dd.cu")
+    cu("fx_kernels_cubature", "fx_kernels_cubature.cu")
     for n in CPLX_DIMS:
         cu("fx_kernels_cplx_n%d" % n, "fx_kernels_cplx.cu", ["-DFX_N=%d" % n])
     for name in ("fiesta_abi", "fx_compiler", "fx_jit"):

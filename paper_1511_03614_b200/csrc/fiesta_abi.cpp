@@ -64,6 +64,7 @@ struct fiesta_ctx {
   DevBuf<int32_t> sel, maps;
   DevBuf<double> partials, hist_part, sums, grid, hist, iter_stats, scratch_d, scratch_d2;
   DevBuf<uint64_t> scratch_u;
+  DevBuf<double> cub_boxes, cub_rec, cub_aux;  // fiesta_integrate_cubature
   DevBuf<unsigned long long> nonfinite;
   DevBuf<fx_result_dev> results;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
@@ -420,6 +421,9 @@ void fiesta_destroy(fiesta_ctx *c) {
   c->scratch_d.release();
   c->scratch_d2.release();
   c->scratch_u.release();
+  c->cub_boxes.release();
+  c->cub_rec.release();
+  c->cub_aux.release();
   c->nonfinite.release();
   c->results.release();
   if (c->fork) cudaEventDestroy(c->fork);
@@ -666,6 +670,7 @@ int fiesta_combine(const fiesta_result *per_sector, int32_t nsectors, int32_t K,
 // planning and the integrate family (second half of this file)
 // ------------------------------------------------------------------------------------------------
 #include "fiesta_abi_integrate.inc"
+#include "fiesta_abi_cubature.inc"
 
 // ------------------------------------------------------------------------------------------------
 // dispatch of the complex kernels, one translation unit per dimension (fx_kernels_cplx.cu -DFX_N=n)

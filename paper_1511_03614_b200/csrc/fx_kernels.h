@@ -161,6 +161,19 @@ cudaError_t fx_launch_transform_points(int rule, const fx_transform_host &tf, co
 cudaError_t fx_launch_eval_dd(const fx_eval_params &prm, cudaStream_t st);  // out[npts][K][hi, lo]
 cudaError_t fx_launch_rescue_real(const fx_integrate_params &prm, int nsectors, cudaStream_t st);
 size_t fx_rescue_smem_bytes(const fx_integrate_params &prm);
+// deterministic cubature (fx_kernels_cubature.cu; R21): Genz-Malik degree-7 rule with embedded degree 5
+#define FX_GM_REC 36  // per-box record: I7[16], |I7-I5|[16], split axis, non-finite node values, sum of the 16 errors, pad
+struct fx_gm_tables {
+  double l2, l3, l5, ratio;  // node radii in units of the half-widths; (l2/l3)^2
+  double w7[5], w5[5];       // weights of the node classes: centre, l2 axis, l3 axis, l3 pairs, corners
+};
+fx_gm_tables fx_gm_make_tables(int n);
+int fx_gm_nodes_per_box(int n);
+// boxes[nboxes][2][n] (centre, half-widths) -> x[nboxes][NN][n]
+cudaError_t fx_launch_gm_nodes(const double *boxes, uint64_t nboxes, int n, double *x, cudaStream_t st);
+// vals[nboxes][NN][ncomp] -> rec[nboxes][FX_GM_REC]; optional i5_out[nboxes][ncomp], d_out[nboxes][n]
+cudaError_t fx_launch_gm_reduce(const double *vals, const double *boxes, uint64_t nboxes, int n, int ncomp, double *rec,
+                                double *i5_out, double *d_out, cudaStream_t st);
 cudaError_t fx_launch_fp64_peak(double *sink_dev, int iters, int blocks, cudaStream_t st);
 
 #endif
