@@ -68,11 +68,13 @@ __global__ void k_gm_nodes(const double *boxes, uint64_t nboxes, int n, int nn, 
   }
 }
 
-// one block per box: I7, |I7 - I5| per component, fourth differences, split axis
+// one block per box: I7, |I7 - I5| per component, fourth differences, split axis.  A thread takes the nodes
+// q = tid, tid + 128, .. with all components of a node at once (they are contiguous); lanes are added by a
+// shuffle tree, the four warps in order: a fixed assignment and order, so the sums are reproducible.
 __global__ void __launch_bounds__(128) k_gm_reduce(const double *vals /*[box][node][ncomp]*/, const double *boxes, int n, int nn,
                                                    int ncomp, fx_gm_tables tb, double *rec /*[box][FX_GM_REC]*/,
                                                    double *i5_out /*[box][ncomp] or NULL*/, double *d_out /*[box][n] or NULL*/) {
-  __shared__ double sh[2][4];
+  __shared__ double sh[2][16][4];
   __shared__ double sh_d[FX_NXMAX];
   const uint64_t b = blockIdx.x;
   const double *v = vals + b * (uint64_t)nn * ncomp;
@@ -82,34 +84,47 @@ __global__ void __launch_bounds__(128) k_gm_reduce(const double *vals /*[box][no
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   double *r = rec + b * FX_GM_REC;
   unsigned bad = 0;
-  for (int c = 0; c < ncomp; ++c) {
-    double s7 = 0.0, s5 = 0.0;
-    for (int q = threadIdx.x; q < nn; q += 128) {  // fixed assignment, fixed order: deterministic
-      int local;
-      const int cls = gm_class(q, n, local);
-      const double f = v[(size_t)q * ncomp + c];
-      bad += isfinite(f) ? 0u : 1u;
-      s7 = fma(tb.w7[cls], f, s7);
-      s5 = fma(tb.w5[cls], f, s5);
-    }
+  double s7[16], s5[16];
 #pragma unroll
-    for (int off = 16; off > 0; off >>= 1) {
-      s7 += __shfl_down_sync(0xffffffffu, s7, off);
-      s5 += __shfl_down_sync(0xffffffffu, s5, off);
+  for (int c = 0; c < 16; ++c) s7[c] = s5[c] = 0.0;
+  for (int q = threadIdx.x; q < nn; q += 128) {
+    int local;
+    const int cls = gm_class(q, n, local);
+    const double w7 = tb.w7[cls], w5 = tb.w5[cls];
+    const double *f = v + (size_t)q * ncomp;
+#pragma unroll
+    for (int c = 0; c < 16; ++c) {
+      if (c < ncomp) {
+        const double fv = f[c];
+        bad += isfinite(fv) ? 0u : 1u;
+        s7[c] = fma(w7, fv, s7[c]);
+        s5[c] = fma(w5, fv, s5[c]);
+      }
     }
-    __syncthreads();
-    if (lane == 0) {
-      sh[0][warp] = s7;
-      sh[1][warp] = s5;
+  }
+#pragma unroll
+  for (int c = 0; c < 16; ++c) {
+    if (c < ncomp) {  // block-uniform
+      double a = s7[c], e = s5[c];
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) {
+        a += __shfl_down_sync(0xffffffffu, a, off);
+        e += __shfl_down_sync(0xffffffffu, e, off);
+      }
+      if (lane == 0) {
+        sh[0][c][warp] = a;
+        sh[1][c][warp] = e;
+      }
     }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-      const double i7 = vol * (((sh[0][0] + sh[0][1]) + sh[0][2]) + sh[0][3]);
-      const double i5 = vol * (((sh[1][0] + sh[1][1]) + sh[1][2]) + sh[1][3]);
-      r[c] = i7;
-      r[16 + c] = fabs(i7 - i5);
-      if (i5_out) i5_out[b * ncomp + c] = i5;
-    }
+  }
+  __syncthreads();
+  if (threadIdx.x < ncomp) {
+    const int c = threadIdx.x;
+    const double i7 = vol * (((sh[0][c][0] + sh[0][c][1]) + sh[0][c][2]) + sh[0][c][3]);
+    const double i5 = vol * (((sh[1][c][0] + sh[1][c][1]) + sh[1][c][2]) + sh[1][c][3]);
+    r[c] = i7;
+    r[16 + c] = fabs(i7 - i5);
+    if (i5_out) i5_out[b * ncomp + c] = i5;
   }
   // fourth divided differences along the axes, summed over the components
   if (threadIdx.x < n) {
@@ -127,7 +142,9 @@ __global__ void __launch_bounds__(128) k_gm_reduce(const double *vals /*[box][no
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) bad += __shfl_down_sync(0xffffffffu, bad, off);
   __shared__ unsigned sh_bad[4];
+  __shared__ double sh_err[16];
   if (lane == 0) sh_bad[warp] = bad;
+  if (threadIdx.x < ncomp) sh_err[threadIdx.x] = r[16 + threadIdx.x];  // this thread wrote it above
   __syncthreads();
   if (threadIdx.x == 0) {
     int axis = 0;
@@ -135,7 +152,7 @@ __global__ void __launch_bounds__(128) k_gm_reduce(const double *vals /*[box][no
       if (sh_d[i] > sh_d[axis]) axis = i;  // ties: the lowest index
     for (int c = ncomp; c < 16; ++c) r[c] = r[16 + c] = 0.0;
     double e = 0.0;
-    for (int c = 0; c < ncomp; ++c) e += r[16 + c];
+    for (int c = 0; c < ncomp; ++c) e += sh_err[c];
     r[32] = (double)axis;
     r[33] = (double)(sh_bad[0] + sh_bad[1] + sh_bad[2] + sh_bad[3]);
     r[34] = e;
