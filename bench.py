@@ -109,7 +109,7 @@ def cpu_baseline(wl, pool, nsec, n_lattice):
     return {"value": evals / dt, "unit": UNIT, "cores": pool.cores, "kind": "oracle",
             "sample": f"{nsec} sectors x {n_lattice} lattice points x {wl.K} orders of {WORKLOAD} "
                       f"(oracle/ as it stands: numpy long double, one process per core), {dt:.1f} s",
-            "value_same_walk_in_double": evals64 / dt64, "double_sample_s": dt64}
+            "sample_s": dt, "value_same_walk_in_double": evals64 / dt64, "double_sample_s": dt64}
 
 
 def run_reference(args):
@@ -336,6 +336,8 @@ def run_b200(args):
         while n_cpu < (1 << 21) and t_cal * (2 * n_cpu / (1 << 12)) < 14.0:
             n_cpu *= 2
         cpu = cpu_baseline(wl_s, pool, 2 * pool.cores, n_cpu)
+        if cpu["sample_s"] < 8.0 and n_cpu < (1 << 21):          # the calibration run carries the pool's start-up
+            cpu = cpu_baseline(wl_s, pool, 2 * pool.cores, 2 * n_cpu)
         pool.close()
 
     # Sectors are independent integrals: ONE program of nsec_full * world sectors is sharded over the ranks
