@@ -469,6 +469,61 @@ def test_lambda_zero_reproduces_real_path(fb, ctx):
     assert np.allclose(b.real[ok], a.real[ok], rtol=1e-11) and np.all(np.abs(b.imag[ok]) <= 1e-11 * np.abs(a.real[ok]))
 
 
+def _box_totals(fb, ctx, terms, integrate):
+    """sum over the front end's integrands, grouped by dimension (one program each) -> (totals [3], sigma [3])"""
+    tot, var = np.zeros(3), np.zeros(3)
+    for d in (1, 2, 3):
+        secs = [SectorText(sector_id=sid, texts=texts) for sid, (dim, texts, _) in enumerate(terms) if dim == d]
+        prog = ctx.compile(secs, d)
+        res = integrate(prog, d)
+        tot += res["re"].sum(axis=0)
+        var += (res["re_err"] ** 2).sum(axis=0)
+        assert np.all(res["n_nonfinite"] == 0)
+        prog.close()
+    return tot, np.sqrt(var)
+
+
+def test_paper_box_example_on_the_gpu(fb, ctx):
+    """PAPER.md:301-313, the massless on-shell box: the 40 integrands of tests/sector_frontend.py (decomposed,
+    pole-subtracted, expanded in eps) through fiesta_compile / fiesta_integrate give the numbers the paper prints
+    within the errors it prints, and the closed form behind them to 1e-9 -- by the lattice rule, by the lattice
+    rule with the mixed-precision rescue switched on (the subtracted integrands are differences over x), and,
+    for the 2- and 3-dimensional integrands, by the deterministic cubature."""
+    import math
+    from conftest import golden
+    from sector_frontend import box_integrands
+    from workloads import korobov_a
+    g = golden("paper_box_example.txt")
+    S, T = int(g["S"]), int(g["T"])
+    exact = [4 / (S * T), -2 * math.log(S * T) / (S * T), (2 * math.log(S) * math.log(T) - 4 * math.pi ** 2 / 3) / (S * T)]
+    terms = box_integrands(S, T)
+
+    def lattice(prog, d):
+        nl = 1 << 14
+        rule = fb.Rule(kind=fb.RULE_LATTICE, n_shifts=8, korobov_a=korobov_a(nl, d) if d > 1 else 1, periodize_r=3)
+        return ctx.integrate(prog, 8 * nl, rule, 20151111)
+
+    tot, sig = _box_totals(fb, ctx, terms, lattice)
+    for k, key in enumerate(("eps_m2", "eps_m1", "eps_0")):
+        assert abs(tot[k] - float(g[key])) <= 3 * float(g[key + "_err"]) + 0.5e-4, (key, tot[k])
+        assert abs(tot[k] - exact[k]) < 1e-9 and sig[k] < 1e-9, (key, tot[k], exact[k], sig[k])
+    ctx.set_mixed(1e-6)
+    try:
+        tot_mixed, _ = _box_totals(fb, ctx, terms, lattice)
+    finally:
+        ctx.set_mixed(0.0)
+    assert np.allclose(tot_mixed, exact, rtol=0, atol=1e-9)
+
+    def cubature(prog, d):
+        if d == 1:
+            return lattice(prog, d)
+        return ctx.integrate_cubature(prog, epsrel=1e-7, epsabs=1e-9, maxeval=1 << 20)[0]
+
+    tot_c, err_c = _box_totals(fb, ctx, terms, cubature)
+    for k in range(3):
+        assert abs(tot_c[k] - exact[k]) <= max(err_c[k], 1e-9) and err_c[k] < 1e-4, (k, tot_c[k], exact[k], err_c[k])
+
+
 def test_bisected_cube_parts_add_up(fb, ctx):
     """PAPER.md:406 BisectionVariables (bisection.py): the parts of a bisected integrand are ordinary sectors --
     per-point parity with the oracle on the rewritten texts -- and their integrals add up: to the closed forms

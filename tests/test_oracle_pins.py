@@ -874,3 +874,42 @@ def test_cubature_rounds_closed_forms_and_bookkeeping():
     small = min(float(np.prod(2 * b["h"])) for b in bx)
     where = [b for b in bx if float(np.prod(2 * b["h"])) == small]
     assert all(abs(float(b["c"][0]) - 0.3) < 0.2 and abs(float(b["c"][1]) - 0.7) < 0.2 for b in where)
+
+
+# ------------------------------------------------------------------ the paper's box example, end to end
+
+def box_closed_form(S, T):
+    """(1/(S T)) [4/eps^2 - 2 (ln S + ln T)/eps + 2 ln S ln T - 4 pi^2/3]: coefficients of eps^-2, eps^-1, eps^0."""
+    return [4 / (S * T), -2 * (math.log(S) + math.log(T)) / (S * T), (2 * math.log(S) * math.log(T) - 4 * math.pi ** 2 / 3) / (S * T)]
+
+
+def test_paper_box_example_end_to_end():
+    """The massless on-shell box of PAPER.md:301-313 through a miniature front end (tests/sector_frontend.py:
+    eq. (2), sector decomposition, pole subtraction, eps expansion -> 40 worker-grammar integrands of 1-3
+    variables) and the oracle's lattice integrator: the numbers the paper prints, within the errors it prints,
+    and the closed form they come from to 1e-9."""
+    from sector_frontend import box_integrands
+    g = golden("paper_box_example.txt")
+    S, T = int(g["S"]), int(g["T"])
+    terms = box_integrands(S, T)
+    assert len(terms) == 40 and sorted({d for d, _, _ in terms}) == [1, 2, 3]
+    tot, var = np.zeros(3), np.zeros(3)
+    for sid, (d, texts, _) in enumerate(terms):
+        nl = {1: 1 << 10, 2: 1 << 12, 3: 1 << 13}[d]
+        gv = P.korobov_genvec(korobov_a(nl, d) if d > 1 else 1, nl, d)
+        val, err = integrate_lattice(SectorSpec(texts, sid), 4 * nl, 4, gv, 3, SEED, rdtype=np.float64)
+        tot += np.asarray(val[:, 0], dtype=float)
+        var += np.asarray(err[:, 0], dtype=float) ** 2
+    exact = box_closed_form(S, T)
+    for k, key in enumerate(("eps_m2", "eps_m1", "eps_0")):
+        assert abs(tot[k] - float(g[key])) <= 3 * float(g[key + "_err"]) + 0.5e-4, (key, tot[k])     # 0.5e-4: the printed digits
+        assert abs(tot[k] - exact[k]) < 1e-9 and math.sqrt(var[k]) < 1e-9, (key, tot[k], exact[k])
+    # other kinematics: the ln S ln T term
+    terms = box_integrands(2, 5)
+    tot = np.zeros(3)
+    for sid, (d, texts, _) in enumerate(terms):
+        nl = {1: 1 << 10, 2: 1 << 12, 3: 1 << 13}[d]
+        gv = P.korobov_genvec(korobov_a(nl, d) if d > 1 else 1, nl, d)
+        val, _ = integrate_lattice(SectorSpec(texts, sid), 4 * nl, 4, gv, 3, SEED, rdtype=np.float64)
+        tot += np.asarray(val[:, 0], dtype=float)
+    assert np.allclose(tot, box_closed_form(2, 5), rtol=0, atol=1e-9)
