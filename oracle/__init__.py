@@ -30,7 +30,8 @@ Pin status (see tests/test_oracle_*.py, all `-m "not gpu"`):
   multiple-precision walk   pinned: closed forms under cancellation, agreement with
   (evaluate_mp, mixed sums)  the long-double walk, 3/2 restored by small_x (R20)
   box example end to end    pinned: the paper's printed numbers
-                            and the closed form, via tests/sector_frontend.py
+                            and the closed form, via tests/sector_frontend.py;
+                            physical-region triangle closed form (complex path)
   cubature (R21)            pinned: degrees of exactness 7 / 5 on every monomial,
                             closed forms, tiling, evaluation count, split axis
   the five BASELINE configs parity unpinned against external truth (random

@@ -185,3 +185,26 @@ def box_integrands(S=3, T=1, orders=(-2, -1, 0)):
                     texts.append(f"{len(vs)};\n0;\n{body};\n|")
                 out.append((len(vs), texts, f"primary {i + 1}, sector {si}, term {ti}"))
     return out
+
+
+def triangle_integrands(s, m2=1):
+    """The one-loop triangle with three equal internal masses m^2 = m2 and two light-like legs, (p1 + p2)^2 = s, in
+    d = 4 (finite), from eq. (2) with l = 1, a = 3:
+
+        J(s) = int d^3x delta(1 - sum x) 1 / (U F),   U = x1 + x2 + x3,   F = m2 U^2 - s x1 x2   (- i0).
+
+    Above the threshold s > 4 m2 F changes sign inside the integration domain: the physical region that
+    the contour deformation of PAPER.md:404 is for.  The three primary sectors need no further decomposition
+    (F = m2 at the origin).  Returns [(texts, deform_f_index)]: blocks of 2 variables with f[1] = U, f[2] = F.
+    """
+    x = sp.symbols("x1:4", positive=True)
+    U = sum(x)
+    F = m2 * U ** 2 - s * x[0] * x[1]
+    out = []
+    for i in range(3):
+        rest = [v for k, v in enumerate(x) if k != i]
+        index = {v: k + 1 for k, v in enumerate(rest)}
+        u_i, f_i = sp.expand(U.subs(x[i], 1)), sp.expand(F.subs(x[i], 1))
+        text = f"2;\n2;\n{to_text(u_i, index)};\n{to_text(f_i, index)};\n1/(f[1]*f[2]);\n|"
+        out.append(([text], 2))
+    return out

@@ -524,6 +524,36 @@ def test_paper_box_example_on_the_gpu(fb, ctx):
         assert abs(tot_c[k] - exact[k]) <= max(err_c[k], 1e-9) and err_c[k] < 1e-4, (k, tot_c[k], exact[k], err_c[k])
 
 
+def test_physical_region_triangle_on_the_gpu(fb, ctx):
+    """The equal-mass triangle above threshold (s = 10 m^2; tests/sector_frontend.py, three 2-dimensional sectors whose F
+    changes sign inside the cube): deformation size from fiesta_select_lambda, then the lattice rule on both
+    tiers and the cubature, against the closed form -(1/(2s)) [ln((1+b)/(1-b)) - i pi]^2."""
+    import math
+    from sector_frontend import triangle_integrands
+    from workloads import korobov_a
+    s_, m2 = 10, 1
+    b = math.sqrt(1 - 4 * m2 / s_)
+    closed = -(1 / (2 * s_)) * (math.log((1 + b) / (1 - b)) - 1j * math.pi) ** 2
+    secs = [SectorText(sector_id=sid, texts=texts, is_complex=True, deform_f_index=fi, lam=1.0)
+            for sid, (texts, fi) in enumerate(triangle_integrands(s_, m2))]
+    prog = ctx.compile(secs, 2)
+    for si in range(3):
+        lam, scan = ctx.select_lambda(prog, si, 1000, 5, lambda_max=1.0, lambda_split=4)
+        assert lam > 0 and all(t["n_bad"] == 0 for t in scan)
+        ctx.set_lambda(prog, si, lam)
+    nl = 1 << 15
+    rule = fb.Rule(kind=fb.RULE_LATTICE, n_shifts=8, korobov_a=korobov_a(nl, 2), periodize_r=3)
+    for tier in (fb.TIER_NATIVE, fb.TIER_INTERPRETER):
+        res = ctx.integrate(prog, 8 * nl, rule, 7, tier=tier)
+        total = complex(res["re"].sum(), res["im"].sum())
+        assert abs(total - closed) < 1e-10 and np.all(res["re_err"] < 1e-10) and np.all(res["im_err"] < 1e-10)
+    cub, _ = ctx.integrate_cubature(prog, epsrel=1e-9, maxeval=1 << 20)
+    total = complex(cub["re"].sum(), cub["im"].sum())
+    assert abs(total - closed) <= max(float(np.sqrt((cub["re_err"] ** 2 + cub["im_err"] ** 2).sum())), 1e-10)
+    assert np.all(cub["re_err"] < 1e-7)
+    prog.close()
+
+
 def test_bisected_cube_parts_add_up(fb, ctx):
     """PAPER.md:406 BisectionVariables (bisection.py): the parts of a bisected integrand are ordinary sectors --
     per-point parity with the oracle on the rewritten texts -- and their integrals add up: to the closed forms

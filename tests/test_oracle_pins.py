@@ -17,7 +17,7 @@ from oracle.deform import (deform, det_lu, differentiate, evaluate_deformed, f_p
 from oracle.evaluate import CLD, LD, evaluate, evaluate_with_magnitude, polygamma_const, PI, EULER_GAMMA
 from oracle.integrate import (SectorSpec, combine_sectors, estimate_from_sums, integrate_lattice, integrate_mc,
                               integrate_vegas, lattice_partial_sums, neumaier_sum, vegas_combine, vegas_refine,
-                              vegas_uniform_grid, exact_sum, ExactSum, mc_partial_sums, vegas_iteration_sums)
+                              vegas_uniform_grid, exact_sum, ExactSum, mc_partial_sums, mc_points, vegas_iteration_sums)
 from oracle.parser import ParseError, parse
 from workloads import korobov_a
 
@@ -913,3 +913,44 @@ def test_paper_box_example_end_to_end():
         val, _ = integrate_lattice(SectorSpec(texts, sid), 4 * nl, 4, gv, 3, SEED, rdtype=np.float64)
         tot += np.asarray(val[:, 0], dtype=float)
     assert np.allclose(tot, box_closed_form(2, 5), rtol=0, atol=1e-9)
+
+
+def triangle_closed_form(s, m2):
+    """J(s) = int_simplex 1/(m2 - s x1 x2 - i0) above the threshold s > 4 m2: -(1/(2s)) [ln((1+b)/(1-b)) - i pi]^2,
+    b = sqrt(1 - 4 m2/s) (the equal-mass scalar triangle with two light-like legs)."""
+    b = math.sqrt(1 - 4 * m2 / s)
+    return -(1 / (2 * s)) * (math.log((1 + b) / (1 - b)) - 1j * math.pi) ** 2
+
+
+def test_physical_region_triangle_closed_form():
+    """A Feynman integral in the physical region, where F changes sign inside the cube (what the contour deformation
+    of PAPER.md:404 is for), in two dimensions: eq. (2) for the equal-mass triangle at s = 10 m^2, three primary
+    sectors from tests/sector_frontend.py, the oracle's deformation (R11) with the deformation size chosen by its
+    lambda scan (R19), against the closed form -- which is checked here, independently, by doing one integration
+    analytically and the other with mpmath."""
+    from sector_frontend import triangle_integrands
+    s, m2 = 10, 1
+    closed = triangle_closed_form(s, m2)
+
+    def inner(x1):         # int_0^(1-x1) dx2 / (m2 - (s + i0) x1 x2) = -ln(1 - (s + i0) x1 (1-x1)/m2) / (s x1)
+        a = 1 - mpmath.mpf(s) * x1 * (1 - x1) / m2
+        return -(mpmath.log(abs(a)) - (1j * mpmath.pi if a < 0 else 0)) / (s * x1)
+
+    b = math.sqrt(1 - 4 * m2 / s)
+    ref = complex(mpmath.quad(inner, [0, (1 - b) / 2, (1 + b) / 2, 1]))
+    assert abs(ref - closed) < 1e-14
+    total = 0j
+    nl = 1 << 13
+    gv = P.korobov_genvec(korobov_a(nl, 2), nl, 2)
+    for sid, (texts, fi) in enumerate(triangle_integrands(s, m2)):
+        probe = SectorSpec(texts, sid, True, fi, 1.0)
+        _, x = mc_points(probe, 5, (1 << 20) - 1, 0, 1000)
+        lam, scan = select_lambda(probe.progs[0], fi, x, 1.0, 4)
+        assert lam is not None and all(t[1] == 0 for t in scan)
+        val, err = integrate_lattice(SectorSpec(texts, sid, True, fi, float(lam)), 4 * nl, 4, gv, 3, SEED)
+        assert float(err[0, 0]) < 1e-10 and float(err[0, 1]) < 1e-10
+        total += complex(float(val[0, 0]), float(val[0, 1]))
+    assert abs(total - closed) < 1e-10
+    # without the deformation the same integrand is not integrable on the real cube
+    val, err = integrate_lattice(SectorSpec(triangle_integrands(s, m2)[0][0], 0, True, 2, 0.0), 4 * nl, 4, gv, 3, SEED)
+    assert not float(err[0, 0]) < 1e-3
