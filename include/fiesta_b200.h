@@ -203,16 +203,17 @@ int fiesta_cubature_rule(fiesta_ctx *ctx, const fiesta_program *prog, int32_t se
 
 /* ---- mixed precision ("MPFR, Native and Mixed (default variant)") ---
  *
- * fiesta_set_mixed: from now on the lattice and plain-MC rules of this context evaluate every point
+ * fiesta_set_mixed: from now on the lattice, plain-MC and Vegas rules of this context evaluate every point
  * with min_k x_k < small_x (the paper's SmallX knob) in double-double
  * arithmetic (two doubles, ~106 bits: this library's stand-in for MPFR) and all other points in
  * double, as before (R20).  The points, their weights and the order of the sums do not
  * change; with no point below small_x the results are bit-identical to small_x = 0.  small_x = 0
  * (the default) switches the mode off; small_x > 1 sends every point through the double-double
- * walk ("-mpfr: evaluate all integration points with the use of MPFR").  Real
- * sectors only: with the mode on, a call that selects a complex sector or uses the Vegas rule
- * fails with FIESTA_E_RULE, and so does FIESTA_TIER_NATIVE (the first phase runs on the interpreter
- * kernels; the default tier choice follows).  Constants enter the double-double walk as the doubles the compiler
+ * walk ("-mpfr: evaluate all integration points with the use of MPFR").  Under the
+ * Vegas rule the decision is taken on the mapped point and the rescued points enter the histogram.
+ * Real sectors only: with the mode on, a call that selects a complex sector fails with
+ * FIESTA_E_RULE, and so does FIESTA_TIER_NATIVE (the first phase runs on the interpreter kernels;
+ * the default tier choice follows).  Constants enter the double-double walk as the doubles the compiler
  * stored.  small_x < 0 or NaN: FIESTA_E_ARG. */
 int fiesta_set_mixed(fiesta_ctx *ctx, double small_x);
 

@@ -327,8 +327,9 @@ def vegas_refine(grid_d, hist_d, alpha):
     return new
 
 
-def vegas_iteration_sums(sec: SectorSpec, grid, npoints, seed, iteration, chunk=1 << 14, rdtype=LD):
+def vegas_iteration_sums(sec: SectorSpec, grid, npoints, seed, iteration, chunk=1 << 14, rdtype=LD, small_x=0.0):
     """S1[K,C], S2[K,C] and histogram h[dim, NB] (sum over orders/components of g^2) of one iteration.
+    `small_x`: the mixed mode of integrand_values (decided on the mapped point x).
 
     All three are exact sums of their terms rounded once (O6, ExactSum): the histogram bin h[d][b]
     is the sum of g^2 over the points whose coordinate d falls in bin b."""
@@ -340,7 +341,7 @@ def vegas_iteration_sums(sec: SectorSpec, grid, npoints, seed, iteration, chunk=
         cnt = min(chunk, npoints - first)
         t, _ = mc_points(sec, seed, iteration, first, cnt, rdtype)
         x, w, b = vegas_map(t, grid, rdtype)
-        vals = integrand_values(sec, x, None, rdtype)
+        vals = integrand_values(sec, x, None, rdtype, small_x)
         g2 = np.zeros(cnt, dtype=rdtype)
         for k in range(sec.K):
             for c, comp in enumerate(_components(vals[k])):
@@ -384,7 +385,7 @@ def vegas_combine(i_it, var_it):
 
 
 def integrate_vegas(sec: SectorSpec, npoints_per_iter, seed, nbins=50, iters=10, alpha=1.5, chunk=1 << 14,
-                    rdtype=LD, trace=None):
+                    rdtype=LD, trace=None, small_x=0.0):
     """Classic Lepage Vegas as restated in DESIGN.md R8.  Returns value, sigma, chi2 [K,C], final grid.
 
     `trace`, if a list, receives per iteration a dict(grid=, s1=, s2=, hist=, I=, var=).
@@ -393,7 +394,7 @@ def integrate_vegas(sec: SectorSpec, npoints_per_iter, seed, nbins=50, iters=10,
     n = rdtype(npoints_per_iter)
     i_list, v_list = [], []
     for it in range(iters):
-        s1, s2, hist = vegas_iteration_sums(sec, grid, npoints_per_iter, seed, it, chunk, rdtype)
+        s1, s2, hist = vegas_iteration_sums(sec, grid, npoints_per_iter, seed, it, chunk, rdtype, small_x)
         i_it = s1 / n
         var_it = (s2 / n - i_it * i_it) / (n - rdtype(1))
         i_list.append(i_it)

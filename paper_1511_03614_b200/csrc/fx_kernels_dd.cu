@@ -4,8 +4,8 @@
 // integration cube where doubles cancel (-SmallX and the other knobs PAPER.md:447,
 // :472; "-mpfr: evaluate all integration points with the use of MPFR").  Here the
 // higher precision is double-double (fx_dd.cuh, ~106 bits) and the decision is the SmallX one: a
-// point with min_k x_k < small_x is "flagged".  The evaluation kernels of both tiers mask flagged
-// points out of their sums (phase 1); fx_rescue_real below makes the same points again, evaluates
+// point with min_k x_k < small_x is "flagged".  The interpreter's evaluation kernels mask flagged
+// points out of their sums and histograms (phase 1); fx_rescue_real below makes the same points again, evaluates
 // the flagged ones by walking the SAME instruction program on (hi, lo) pairs, and adds them to the
 // same per-block partial records before the chunk reduction runs (phase 2).  The points, their
 // weights and the order of the sums stay those of phase 1; only f(x) is computed more precisely.
@@ -134,20 +134,22 @@ struct RescueSink {
   double *acc;  // &acc[0][tid], slot stride FX_THREADS
   double W;
   unsigned nonfinite;
+  double h2;    // sum over the orders of g^2: what the Vegas histogram collects
   __device__ __forceinline__ void operator()(int k, dd a) {
     const double g = W * a.hi;  // the value rounded to double, as the sums are
     nonfinite += isfinite(g) ? 0u : 1u;
     acc[(2 * k) * FX_THREADS] += g;
     acc[(2 * k + 1) * FX_THREADS] = fma(g, g, acc[(2 * k + 1) * FX_THREADS]);
+    h2 = fma(g, g, h2);
   }
 };
 
 constexpr int FX_RQ = 64;  // entries of a warp's queue of flagged point indices
 
 struct fx_rescue_smem {
-  uint32_t prog, mem, acc, delta, queue, wsum, rec, total;
+  uint32_t prog, mem, acc, delta, queue, wsum, rec, grid, hist, total;
 };
-__host__ __device__ inline fx_rescue_smem fx_rescue_layout(int prog_ins, int mem_doubles) {
+__host__ __device__ inline fx_rescue_smem fx_rescue_layout(int prog_ins, int mem_doubles, int dim, int nbins, bool vegas) {
   fx_rescue_smem L;
   uint32_t o = 0;
   L.prog = o;
@@ -164,18 +166,22 @@ __host__ __device__ inline fx_rescue_smem fx_rescue_layout(int prog_ins, int mem
   o += FX_ACC_SLOTS * (FX_THREADS / 32) * 8u;
   L.rec = o;
   o += FX_ACC_SLOTS * 8u;
+  L.grid = o;
+  o += vegas ? (uint32_t)dim * (nbins + 1) * 8u : 0u;
+  L.hist = o;
+  o += vegas ? (FX_THREADS / 32) * (uint32_t)dim * nbins * 8u : 0u;  // one histogram per warp, as in phase 1
   L.total = o;
   return L;
 }
 
 template <int NX, int RULE>
 __global__ void __launch_bounds__(FX_THREADS) fx_rescue_real(const __grid_constant__ fx_integrate_params prm) {
-  static_assert(RULE != FIESTA_RULE_VEGAS, "lattice and plain MC only");
+  constexpr bool vegas = RULE == FIESTA_RULE_VEGAS;
   extern __shared__ __align__(16) unsigned char smem[];
   const fx_block_id id = fx_block_coords(prm);
   const fx_sector_dev sec = prm.sectors[prm.sel[id.sel_idx]];
   const int dim = prm.dim;
-  const fx_rescue_smem L = fx_rescue_layout(prm.prog_ins_max, prm.mem_doubles);
+  const fx_rescue_smem L = fx_rescue_layout(prm.prog_ins_max, prm.mem_doubles, dim, prm.nbins, vegas);
   fx_ins *sh_prog = reinterpret_cast<fx_ins *>(smem + L.prog);
   double *sh_mem = reinterpret_cast<double *>(smem + L.mem);
   double *sh_acc = reinterpret_cast<double *>(smem + L.acc);
@@ -183,9 +189,11 @@ __global__ void __launch_bounds__(FX_THREADS) fx_rescue_real(const __grid_consta
   uint64_t *sh_queue = reinterpret_cast<uint64_t *>(smem + L.queue) + (threadIdx.x >> 5) * FX_RQ;
   double *sh_wsum = reinterpret_cast<double *>(smem + L.wsum);
   double *sh_rec = reinterpret_cast<double *>(smem + L.rec);
+  double *sh_grid = reinterpret_cast<double *>(smem + L.grid);
+  double *sh_hist = reinterpret_cast<double *>(smem + L.hist);
 
   fx_copy_program(sh_prog, prm.arena + sec.main_off, sec.main_len);
-  fx_block_setup(prm, dim, (uint32_t)sec.sector_id, id.r, id.sel_idx, sh_delta, nullptr, nullptr);
+  fx_block_setup(prm, dim, (uint32_t)sec.sector_id, id.r, id.sel_idx, sh_delta, sh_grid, sh_hist);
   const int nslots = 2 * sec.K;
   for (int s = 0; s < nslots; ++s) sh_acc[s * FX_THREADS + threadIdx.x] = 0.0;
   __syncthreads();
@@ -198,21 +206,27 @@ __global__ void __launch_bounds__(FX_THREADS) fx_rescue_real(const __grid_consta
 
   // one queued point per lane: made again from its index, evaluated in double-double
   auto drain = [&](unsigned n) {
+    uint32_t bins[(NX + 3) / 4][1];
+    double h2[1] = {0.0};
+#pragma unroll
+    for (int q = 0; q < (NX + 3) / 4; ++q) bins[q][0] = 0;
     if (lane < n) {
       double x[NX][1], xbar[NX][1], W[1];
-      uint32_t bins[(NX + 3) / 4][1];
       unsigned valid;
-      fx_make_points<RULE, NX, 1>(prm, dim, (uint32_t)sec.sector_id, sh_delta, nullptr, sh_queue[lane], c1, x, xbar, W, valid, bins);
+      fx_make_points<RULE, NX, 1>(prm, dim, (uint32_t)sec.sector_id, sh_delta, sh_grid, sh_queue[lane], c1, x, xbar, W, valid, bins);
       dd R[FX_NR];
 #pragma unroll
       for (int k = 0; k < FX_NR; ++k) R[k] = dd_from(0.5);
 #pragma unroll
       for (int k = 0; k < NX; ++k) R[k] = dd_from(x[k][0]);
-      RescueSink sink{sh_acc + threadIdx.x, W[0], 0u};
+      RescueSink sink{sh_acc + threadIdx.x, W[0], 0u, 0.0};
       fx_run_dd(sh_prog, R, M, sink);
       nonfinite += sink.nonfinite;
+      h2[0] = sink.h2;
     }
     __syncwarp();
+    // Vegas: the rescued points' g^2 go to the warp's histogram by the same warp-collective, fixed-order update as in phase 1
+    if constexpr (vegas) fx_hist_points<NX, 1>(sh_hist, dim, prm.nbins, lane < n ? 1u : 0u, bins, h2);
   };
 
   // the same trip count for every thread: the queue is a warp-collective structure
@@ -221,7 +235,7 @@ __global__ void __launch_bounds__(FX_THREADS) fx_rescue_real(const __grid_consta
     double x[NX][1], xbar[NX][1], W[1];
     uint32_t bins[(NX + 3) / 4][1];
     unsigned valid;
-    fx_make_points<RULE, NX, 1>(prm, dim, (uint32_t)sec.sector_id, sh_delta, nullptr, j, c1, x, xbar, W, valid, bins);
+    fx_make_points<RULE, NX, 1>(prm, dim, (uint32_t)sec.sector_id, sh_delta, sh_grid, j, c1, x, xbar, W, valid, bins);
     const bool flag = j < c1 && fx_flag_mask<NX, 1>(x, dim, prm.small_x);  // (fx_make_points cleared the flagged bit of `valid`)
     const unsigned m = __ballot_sync(0xffffffffu, flag);
     if (flag) sh_queue[queued + __popc(m & ((1u << lane) - 1u))] = j;
@@ -244,6 +258,15 @@ __global__ void __launch_bounds__(FX_THREADS) fx_rescue_real(const __grid_consta
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) nonfinite += __shfl_down_sync(0xffffffffu, nonfinite, off);
   if (lane == 0 && nonfinite) atomicAdd(prm.nonfinite + id.sel_idx, (unsigned long long)nonfinite);
+  if constexpr (vegas) {  // the warps' histograms in warp order, added to the record phase 1 wrote for this block
+    const int cells = dim * prm.nbins;
+    double *h = prm.hist_part + ((size_t)(id.sel_idx - prm.batch_base) * prm.nchunks + id.chunk) * cells;
+    for (int i = threadIdx.x; i < cells; i += blockDim.x) {
+      double v = 0.0;
+      for (int w = 0; w < FX_THREADS / 32; ++w) v += sh_hist[w * cells + i];
+      h[i] += v;
+    }
+  }
 }
 
 }  // namespace
@@ -261,11 +284,12 @@ cudaError_t fx_launch_eval_dd(const fx_eval_params &prm, cudaStream_t st) {
   return cudaGetLastError();
 }
 
-size_t fx_rescue_smem_bytes(const fx_integrate_params &prm) { return fx_rescue_layout(prm.prog_ins_max, prm.mem_doubles).total; }
+size_t fx_rescue_smem_bytes(const fx_integrate_params &prm) {
+  return fx_rescue_layout(prm.prog_ins_max, prm.mem_doubles, prm.dim, prm.nbins, prm.rule == FIESTA_RULE_VEGAS).total;
+}
 
 // prm.mem_doubles = 2 * max n_mem_main * FX_THREADS; launch_map / sel_base as for the evaluation kernels
 cudaError_t fx_launch_rescue_real(const fx_integrate_params &prm, int nsectors, cudaStream_t st) {
-  if (prm.rule == FIESTA_RULE_VEGAS) return cudaErrorInvalidValue;
   const size_t smem = fx_rescue_smem_bytes(prm);
   const unsigned grid = (unsigned)((size_t)nsectors * prm.n_shifts * prm.nchunks);
   cudaError_t e;
@@ -277,7 +301,8 @@ cudaError_t fx_launch_rescue_real(const fx_integrate_params &prm, int nsectors, 
 #define FX_LAUNCH(NX)                                                        \
   {                                                                          \
     if (prm.rule == FIESTA_RULE_LATTICE) FX_LAUNCH2(NX, FIESTA_RULE_LATTICE) \
-    else FX_LAUNCH2(NX, FIESTA_RULE_MC)                                      \
+    else if (prm.rule == FIESTA_RULE_MC) FX_LAUNCH2(NX, FIESTA_RULE_MC)      \
+    else FX_LAUNCH2(NX, FIESTA_RULE_VEGAS)                                   \
   }
   if (prm.dim <= 4) FX_LAUNCH(4)
   else if (prm.dim <= 8) FX_LAUNCH(8)

@@ -145,6 +145,36 @@ def test_mixed_sums_against_oracle(fb, ctx, kind, tier):
         prog.close()
 
 
+def test_mixed_vegas_iteration_against_oracle(fb, ctx):
+    """Vegas with the rescue on: one iteration on a given uneven grid -- sums and the g^2 histogram, bin by bin, against
+    the oracle's mixed iteration -- and a full run that reaches the closed form 3/2."""
+    small_x = 0.02
+    s = SectorText(sector_id=6, texts=[CANCEL])
+    prog = ctx.compile([s], 2)
+    sec = spec(s)
+    rule = fb.Rule(kind=fb.RULE_VEGAS, vegas_bins=16, vegas_iters=5, vegas_alpha=1.5)
+    rng = np.random.default_rng(4)
+    w = rng.random((2, 16)).astype(LD) ** 2 + LD(1e-2)
+    grid = np.concatenate([np.zeros((2, 1), dtype=LD), np.cumsum(w, axis=1) / np.sum(w, axis=1)[:, None]], axis=1)
+    grid[:, -1] = 1
+    gridf = grid.astype(np.float64)
+    npts = 6007
+    ctx.set_mixed(small_x)
+    try:
+        s1, s2, hist = OI.vegas_iteration_sums(sec, gridf.astype(LD), npts, 21, 2, small_x=small_x)
+        sums, h = ctx.vegas_iteration(prog, 0, npts, rule, 21, 2, gridf)
+        assert np.allclose(sums[..., 0], s1.astype(float), rtol=1e-10)
+        assert np.allclose(sums[..., 1], s2.astype(float), rtol=1e-10)
+        hf = hist.astype(float)
+        assert np.allclose(h, hf, rtol=1e-10, atol=1e-13 * hf.max())
+        assert np.allclose(h.sum(axis=1), sums[0, 0, 1], rtol=1e-12)
+        res = ctx.integrate(prog, 20000, rule, 22)[0]
+        assert abs(res["re"][0] - 1.5) <= 4 * res["re_err"][0] and res["re_err"][0] < 0.01 and res["n_nonfinite"][0] == 0
+    finally:
+        ctx.set_mixed(0.0)
+        prog.close()
+
+
 def test_mixed_mode_with_nothing_flagged_is_bit_identical(fb, ctx):
     """small_x below every coordinate: phase 2 finds no point, the sums are the bits of the plain run; and
     small_x > 1 (every point through the double-double walk, the paper's -mpfr) agrees to FP64 accuracy."""
@@ -177,14 +207,9 @@ def test_mixed_mode_refuses_what_it_does_not_cover(fb, ctx):
     ctx.set_mixed(1e-3)
     try:
         with pytest.raises(fb.FiestaError):
-            ctx.partial_sums(prog, wl.npoints, fb.Rule.from_workload(wl), wl.seed)      # complex sector
+            ctx.partial_sums(prog, wl.npoints, fb.Rule.from_workload(wl), wl.seed)      # complex sector: not covered
         with pytest.raises(fb.FiestaError):
             ctx.eval_points_dd(prog, 0, np.full((1, wl.dim), 0.5))
-        real = make_workload("C5", nsectors=1, npoints=1 << 12)
-        p2 = ctx.compile(real.sectors, real.dim)
-        with pytest.raises(fb.FiestaError):
-            ctx.integrate(p2, real.npoints, fb.Rule.from_workload(real), real.seed)     # Vegas
-        p2.close()
         with pytest.raises(fb.FiestaError):
             ctx.set_mixed(-1.0)
     finally:
