@@ -176,6 +176,24 @@ int fiesta_eval_points(fiesta_ctx *ctx, const fiesta_program *prog, int32_t sect
 int fiesta_eval_points_tier(fiesta_ctx *ctx, const fiesta_program *prog, int32_t sector, int32_t tier,
                             const double *x_host, uint64_t npts, double *out_host);
 
+/* ---- few, huge sectors: the shifts of the lattice rule split over ranks ----------
+ *
+ * fiesta_partial_sums_shifts: fiesta_partial_sums for the shifts shift_first .. shift_first +
+ * shift_count - 1 of the rule's n_shifts only (lattice rule; npoints is still the rule's total,
+ * n_shifts x N_L).  sums_host[nsel][shift_count][K][C][2].  A shift's sums do not depend on which
+ * other shifts a call computes: the rows are, bit for bit, those of the full call.
+ * fiesta_last_nonfinite: the per-sector counts of NaN / Inf values of the last integrate-family call.
+ * fiesta_estimate_from_sums: the estimator (R5) on the device from per-shift sums in the
+ * layout of fiesta_partial_sums ([nsel][n_shifts][K][C][2]; all sectors with the same K), e.g. the
+ * rows the ranks have exchanged; nonfinite_host[nsel] may be NULL (zeros).  out[nsel][K]. */
+int fiesta_partial_sums_shifts(fiesta_ctx *ctx, const fiesta_program *prog, const int32_t *sectors, int32_t nsel,
+                               int32_t dim, uint64_t npoints, const fiesta_rule *rule, uint64_t seed, int32_t tier,
+                               int32_t shift_first, int32_t shift_count, double *sums_host);
+int fiesta_last_nonfinite(fiesta_ctx *ctx, int32_t nsel, uint64_t *counts_host);
+int fiesta_estimate_from_sums(fiesta_ctx *ctx, const fiesta_program *prog, const int32_t *sectors, int32_t nsel,
+                              int32_t n_shifts, uint64_t n_per_shift, const double *sums_host,
+                              const uint64_t *nonfinite_host, fiesta_result *out);
+
 /* ---- deterministic integrator (PAPER.md:412 `CurrentIntegrator -> cuhreCuba`) ------
  *
  * A Cuhre-like globally adaptive cubature on the same evaluator (R21): the degree-7 rule of

@@ -88,6 +88,9 @@ _SIGNATURES = {
     "fiesta_program_set_lambda": (C.c_int, [_VP, _VP, _I32, C.c_double]),
     "fiesta_integrate_cubature": (C.c_int, [_VP, _VP, _VP, _I32, C.c_double, C.c_double, _U64, _I32, _VP, _VP]),
     "fiesta_cubature_rule": (C.c_int, [_VP, _VP, _I32, _I32, _VP, _U64, _VP, _VP, _VP, _VP]),
+    "fiesta_partial_sums_shifts": (C.c_int, [_VP, _VP, _VP, _I32, _I32, _U64, C.POINTER(_Rule), _U64, _I32, _I32, _I32, _VP]),
+    "fiesta_last_nonfinite": (C.c_int, [_VP, _I32, _VP]),
+    "fiesta_estimate_from_sums": (C.c_int, [_VP, _VP, _VP, _I32, _I32, _U64, _VP, _VP, _VP]),
     "fiesta_set_mixed": (C.c_int, [_VP, C.c_double]),
     "fiesta_eval_points_dd": (C.c_int, [_VP, _VP, _I32, _VP, _U64, _VP]),
 }
@@ -366,6 +369,31 @@ class Context:
         r, keep = rule._c()
         self._check(self.lib.fiesta_partial_sums_tier(self.handle, prog.handle, _ptr(sel), nsel, prog.dim, int(npoints),
                                                       C.byref(r), int(seed), int(tier), _ptr(out)))
+        return out
+
+    def partial_sums_shifts(self, prog, npoints, rule, seed, shift_first, shift_count, sectors=None, tier=TIER_ANY):
+        """The rows shift_first .. shift_first + shift_count - 1 of partial_sums -> ([nsectors][count][K][C][2],
+        per-sector non-finite counts)."""
+        sel, nsel, idx = self._sel(prog, sectors)
+        K, cc = prog.K[idx[0]], 2 if prog.is_complex[idx[0]] else 1
+        out = np.zeros((nsel, int(shift_count), K, cc, 2), dtype=np.float64)
+        r, keep = rule._c()
+        self._check(self.lib.fiesta_partial_sums_shifts(self.handle, prog.handle, _ptr(sel), nsel, prog.dim, int(npoints),
+                                                        C.byref(r), int(seed), int(tier), int(shift_first), int(shift_count),
+                                                        _ptr(out)))
+        nf = np.zeros(nsel, dtype=np.uint64)
+        self._check(self.lib.fiesta_last_nonfinite(self.handle, nsel, _ptr(nf)))
+        return out, nf
+
+    def estimate_from_sums(self, prog, sums, n_per_shift, nonfinite=None, sectors=None, allow_nonfinite=False):
+        """sums [nsectors][R][K][C][2] -> record array [nsectors][K] (the estimator of fiesta_integrate, on the device)."""
+        sel, nsel, idx = self._sel(prog, sectors)
+        sums = np.ascontiguousarray(sums, dtype=np.float64)
+        R = sums.shape[1]
+        out = np.zeros((nsel, prog.K[idx[0]]), dtype=RESULT_DTYPE)
+        nf = None if nonfinite is None else np.ascontiguousarray(nonfinite, dtype=np.uint64)
+        self._check(self.lib.fiesta_estimate_from_sums(self.handle, prog.handle, _ptr(sel), nsel, R, int(n_per_shift), _ptr(sums),
+                                                       _ptr(nf), _ptr(out)), allow_nonfinite)
         return out
 
     def chunk_sums(self, prog, npoints, rule, seed, sectors=None, tier=TIER_ANY):

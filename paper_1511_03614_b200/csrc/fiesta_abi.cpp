@@ -164,6 +164,7 @@ struct Plan {
   size_t smem = 0;
   int mem_dd = 0;             // mixed precision: spill doubles per block of the double-double walk
   bool no_mixed = false;      // a caller that never runs phase 2 (fiesta_test_f)
+  int shift_first = 0, shift_count = 0;  // lattice: only shifts [first, first + count) of the rule's R (0: all)
 };
 
 int ilog2_exact(uint64_t n) {

@@ -227,7 +227,7 @@ __device__ __forceinline__ void fx_block_setup(const fx_integrate_params &prm, i
   if (threadIdx.x < (FX_NXMAX + 1) / 2) {
     uint64_t te = 0, to = 0;
     if (prm.rule == FIESTA_RULE_LATTICE)
-      philox_t_pair_rk(prm.philox_rk, sector_id, FX_TAG_SHIFT, (uint32_t)r, 0ull, threadIdx.x, te, to);
+      philox_t_pair_rk(prm.philox_rk, sector_id, FX_TAG_SHIFT, (uint32_t)(prm.shift_base + r), 0ull, threadIdx.x, te, to);
     sh_delta[2 * threadIdx.x] = te;
     sh_delta[2 * threadIdx.x + 1] = to;
   }

@@ -73,6 +73,7 @@ struct fx_integrate_params {
   // mixed precision (fiesta_set_mixed; R20): points with some x_k < small_x are left out of the sums
   // here and evaluated in double-double by fx_launch_rescue_real.  0: off.
   double small_x;
+  int32_t shift_base;        // lattice: the block's shift r stands for shift shift_base + r of the rule (a rank's share of the shifts)
 };
 
 // position in the selection of the sector a block works on

@@ -69,3 +69,62 @@ def max_over_ranks(value, dist=None, device="cpu"):
     t = torch.tensor([float(value)], dtype=torch.float64, device=device)
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return float(t.item())
+
+
+def split_shifts(n_shifts, world_size):
+    """(first, count) per rank: the rule's shifts dealt out in contiguous, near-equal shares (count may be 0)."""
+    base, extra = divmod(int(n_shifts), int(world_size))
+    out, first = [], 0
+    for r in range(world_size):
+        cnt = base + (1 if r < extra else 0)
+        out.append((first, cnt))
+        first += cnt
+    return out
+
+
+def integrate_split_shifts(ctx, prog, npoints, rule, seed, sectors=None, dist=None, device="cpu"):
+    """Few, huge sectors: every rank integrates ALL selected sectors, but only its share of the lattice rule's
+    random shifts (the shifts are independent estimates of the same integral: no exchange until the end); one
+    all_gather of the per-shift sums (KBs), then every rank runs the estimator on the device.  The result is,
+    bit for bit, fiesta_integrate's on one GPU: a shift's sums do not depend on the rank that made them.
+
+    ctx: binding.Context; prog: a Program compiled on every rank from the same sectors; rule: lattice."""
+    world = dist.get_world_size() if (dist is not None and dist.is_initialized()) else 1
+    rank = dist.get_rank() if world > 1 else 0
+    R = int(rule.n_shifts)
+    shares = split_shifts(R, world)
+    first, cnt = shares[rank]
+    nsel = prog.nsectors if sectors is None else len(sectors)
+    mine = nf = None
+    if cnt > 0:
+        mine, nf = ctx.partial_sums_shifts(prog, npoints, rule, seed, first, cnt, sectors=sectors)
+    if world == 1:
+        return ctx.estimate_from_sums(prog, mine, npoints // R, nf, sectors=sectors, allow_nonfinite=True)
+    import torch
+    # fixed-size buffers padded to the largest share; a rank without a shift (more ranks than shifts) sends zeros
+    row = None if mine is None else int(np.prod(mine.shape[2:]))
+    rows = [None] * world
+    dist.all_gather_object(rows, row)
+    row = next(v for v in rows if v is not None)
+    cap = max(c for _, c in shares)
+    buf = np.zeros(nsel * cap * row + nsel, dtype=np.float64)
+    if cnt > 0:
+        buf[:nsel * cnt * row] = mine.reshape(-1)
+        buf[nsel * cap * row:] = nf.astype(np.float64)         # counts < 2^53
+    t = torch.from_numpy(buf).to(device)
+    got = [torch.empty_like(t) for _ in range(world)]
+    dist.all_gather(got, t)
+    tail = mine.shape[2:] if mine is not None else None
+    tails = [None] * world
+    dist.all_gather_object(tails, tail)
+    tail = next(v for v in tails if v is not None)
+    full = np.zeros((nsel, R) + tuple(tail), dtype=np.float64)
+    nf_all = np.zeros(nsel, dtype=np.uint64)
+    for r, g in enumerate(got):
+        f0, c = shares[r]
+        if c == 0:
+            continue
+        b = g.cpu().numpy()
+        full[:, f0:f0 + c] = b[:nsel * c * row].reshape((nsel, c) + tuple(tail))
+        nf_all += b[nsel * cap * row:].astype(np.uint64)
+    return ctx.estimate_from_sums(prog, full, npoints // R, nf_all, sectors=sectors, allow_nonfinite=True)

@@ -554,6 +554,34 @@ def test_physical_region_triangle_on_the_gpu(fb, ctx):
     prog.close()
 
 
+def test_shifts_split_over_ranks_give_identical_bits(fb, ctx):
+    """SURVEY 8(e), few huge sectors: the shifts of the lattice rule dealt to ranks.  What rank i of 3 would compute
+    (fiesta_partial_sums_shifts) is, bit for bit, rows of the full call on both tiers -- real and complex sectors --
+    and fiesta_estimate_from_sums on the gathered rows is fiesta_integrate's result; world size 1 of
+    sharding.integrate_split_shifts as well."""
+    from paper_1511_03614_b200.sharding import integrate_split_shifts, split_shifts
+    for name, npts in (("C3", 1 << 15), ("C4", 1 << 13)):
+        wl = make_workload(name, nsectors=2, npoints=npts, n_shifts=8)
+        prog = ctx.compile(wl.sectors, wl.dim)
+        rule = fb.Rule.from_workload(wl)
+        for tier in (fb.TIER_NATIVE, fb.TIER_INTERPRETER):
+            full = ctx.partial_sums(prog, wl.npoints, rule, wl.seed, tier=tier)
+            rows = np.zeros_like(full)
+            for first, cnt in split_shifts(8, 3):
+                part, nf = ctx.partial_sums_shifts(prog, wl.npoints, rule, wl.seed, first, cnt, tier=tier)
+                rows[:, first:first + cnt] = part
+                assert np.all(nf == 0)
+            assert rows.tobytes() == full.tobytes()
+        direct = ctx.integrate(prog, wl.npoints, rule, wl.seed)
+        assert ctx.estimate_from_sums(prog, rows, wl.n_lattice).tobytes() == direct.tobytes()
+        assert integrate_split_shifts(ctx, prog, wl.npoints, rule, wl.seed).tobytes() == direct.tobytes()
+        with pytest.raises(fb.FiestaError):
+            ctx.partial_sums_shifts(prog, wl.npoints, rule, wl.seed, 6, 3)          # beyond the rule's 8 shifts
+        with pytest.raises(fb.FiestaError):
+            ctx.partial_sums_shifts(prog, wl.npoints, fb.Rule(kind=fb.RULE_MC), wl.seed, 0, 1)
+        prog.close()
+
+
 def test_bisected_cube_parts_add_up(fb, ctx):
     """PAPER.md:406 BisectionVariables (bisection.py): the parts of a bisected integrand are ordinary sectors --
     per-point parity with the oracle on the rewritten texts -- and their integrals add up: to the closed forms

@@ -263,3 +263,63 @@ def test_pool_resubmits_the_work_of_frozen_ranks(tmp_path, lib):
     p = IntegrationPool(ctx, secs, 1, rule, 1000, 9, store_path=path2, group=4, costs=costs, dist=_StubDist(2, 3))
     assert p.run_to_completion(stale_after=0.0, poll=0.01, timeout=5.0)
     assert sorted(s for g in ctx.integrated for s in g) == [100 + i for i in range(20)] and p.n_adopted == 20 - len(p.my_local)
+
+
+# ------------------------------------------------------------------ few, huge sectors: shifts split over ranks
+
+_GLOO_SHIFTS = r"""
+import sys
+import numpy as np
+import torch.distributed as dist
+sys.path.insert(0, {root!r})
+from paper_1511_03614_b200.sharding import integrate_split_shifts, split_shifts
+from paper_1511_03614_b200.binding import Rule
+world = {world}
+dist.init_process_group("gloo", init_method="tcp://127.0.0.1:{port}", rank=int(sys.argv[1]), world_size=world)
+
+class Prog:
+    nsectors = 3
+
+class Ctx:
+    '''stands in for binding.Context: the sums of (sector, shift) are a fixed function of both'''
+    def __init__(self): self.asked = []
+    def partial_sums_shifts(self, prog, npoints, rule, seed, first, count, sectors=None, tier=-1):
+        self.asked.append((first, count))
+        out = np.zeros((3, count, 2, 1, 2))
+        for s in range(3):
+            for r in range(count):
+                out[s, r] = 1000 * s + 10 * (first + r) + np.arange(4).reshape(2, 1, 2)
+        return out, np.array([first, 0, count], dtype=np.uint64)
+    def estimate_from_sums(self, prog, sums, n_per_shift, nonfinite=None, sectors=None, allow_nonfinite=False):
+        return sums, nonfinite, n_per_shift
+
+R = {R}
+ctx = Ctx()
+sums, nf, nps = integrate_split_shifts(ctx, Prog(), 8 * R, Rule(kind=0, n_shifts=R), 1, dist=dist)
+shares = split_shifts(R, world)
+assert ctx.asked == ([shares[dist.get_rank()]] if shares[dist.get_rank()][1] else [])
+assert sums.shape == (3, R, 2, 1, 2) and nps == 8
+for s in range(3):
+    for r in range(R):
+        assert np.array_equal(sums[s, r], 1000 * s + 10 * r + np.arange(4).reshape(2, 1, 2))
+assert nf.tolist() == [sum(f for f, c in shares if c), 0, R]
+print("ok")
+dist.barrier()
+dist.destroy_process_group()
+"""
+
+
+@pytest.mark.parametrize("world,R", [(2, 8), (3, 2)])
+def test_shifts_split_over_ranks_gloo(tmp_path, world, R):
+    """sharding.integrate_split_shifts: every rank asks for its share of the shifts only, the gathered rows are in
+    shift order on every rank, non-finite counts add up; also with more ranks than shifts."""
+    from paper_1511_03614_b200.sharding import split_shifts
+    assert split_shifts(8, 3) == [(0, 3), (3, 3), (6, 2)] and split_shifts(2, 3) == [(0, 1), (1, 1), (2, 0)]
+    script = tmp_path / "s.py"
+    port = 31500 + (os.getpid() + 7 * world) % 2000
+    script.write_text(_GLOO_SHIFTS.format(root=ROOT, port=port, world=world, R=R))
+    procs = [subprocess.Popen([sys.executable, str(script), str(r)], stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True)
+             for r in range(world)]
+    outs = [p.communicate(timeout=180) for p in procs]
+    for p, (o, e) in zip(procs, outs):
+        assert p.returncode == 0 and "ok" in o, e[-2000:]
