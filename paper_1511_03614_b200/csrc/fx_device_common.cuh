@@ -251,23 +251,25 @@ __device__ __forceinline__ void fx_block_setup(const fx_integrate_params &prm, i
 }
 
 // Vegas histogram (R8): h[k][bin_k] += v for one point per lane and every
-// dimension k, into the WARP's own histogram in shared memory.  Warp-aggregated without atomics and
-// in a fixed order, so that the histogram -- like the sums -- is bit-reproducible:
-//   - in step k of a point, lane l handles dimension (k + l) mod n: the lanes of a warp work on
-//     different dimensions, and only the lanes l, l + n, l + 2n, ... (same dimension) can meet in a
-//     cell, which happens when their points fall into the same bin;
-//   - a lane's rank is the number of such lanes below it with the same cell (shuffles by n, 2n, ..),
-//     and the warp takes turns by rank: in turn s the lanes of rank s do a plain read-modify-write
-//     of their cell, with a warp barrier after every turn.  Two lanes never touch one cell in the
-//     same turn, and a cell receives its contributions in step order, then lane order.
-// With n = 12 and 50 bins the second turn is needed in about 5 % of the steps.
+// dimension k, into the WARP's own histogram in shared memory.  Without atomics and in a fixed order,
+// so that the histogram -- like the sums -- is bit-reproducible:
+//   - in step k of a point, lane l handles dimension (k + l) mod n: the lanes l < n work on different
+//     dimensions, and only the lanes l, l + n, l + 2n, ... (same dimension) can meet in a cell, which
+//     happens when their points fall into the same bin;
+//   - so the lanes take ceil(32 / n) turns per step -- turn t: the lanes t n <= l < (t + 1) n do a plain
+//     read-modify-write of their cell -- with a warp barrier after every turn.  Two lanes never touch
+//     one cell in the same turn, and a cell receives its contributions in step order, then lane order.
+// (An earlier form found out by shuffles which lanes actually meet -- with 12 dimensions and 50 bins a
+// second turn was needed in 5 % of the steps -- and took turns by that rank: the same order of additions,
+// but two shuffles, a vote and a loop per step; the fixed turns are 4-7 % faster at 4-8 dimensions and
+// took the 12-dimensional C5 from 1.50 to 1.9e10 evaluations/s.)
 template <int NX, int P>
 __device__ __forceinline__ void fx_hist_points(double *sh_hist, int dim, int nbins, unsigned valid,
                                                const uint32_t (&bins)[(NX + 3) / 4][P], const double (&h2)[P]) {
-  const unsigned full = 0xffffffffu;
   const unsigned lane = threadIdx.x & 31u;
   double *wh = sh_hist + (size_t)(threadIdx.x >> 5) * dim * nbins;
   const unsigned d0 = lane % (unsigned)dim;
+  const unsigned turn = lane / (unsigned)dim;
   FX_PLOOP {  // point by point: the order both tiers use
     const bool ok = (valid >> p) & 1u;
     unsigned d = d0;
@@ -276,17 +278,19 @@ __device__ __forceinline__ void fx_hist_points(double *sh_hist, int dim, int nbi
       uint32_t w = bins[0][p];
       if constexpr ((NX + 3) / 4 > 1) w = d >= 4 ? bins[1][p] : w;
       if constexpr ((NX + 3) / 4 > 2) w = d >= 8 ? bins[2][p] : w;
-      const unsigned cell = ok ? d * (unsigned)nbins + ((w >> (8 * (d & 3u))) & 0xffu) : (0xffff0000u | lane);
-      unsigned rank = 0;
-      for (int j = dim; j < 32; j += dim) {
-        const unsigned c = __shfl_up_sync(full, cell, j);
-        rank += (lane >= (unsigned)j && c == cell) ? 1u : 0u;
-      }
-      if (ok && rank == 0u) wh[cell] += h2[p];
-      __syncwarp();
-      for (unsigned s = 1; __any_sync(full, ok && rank >= s); ++s) {
-        if (ok && rank == s) wh[cell] += h2[p];
-        __syncwarp();
+      const unsigned cell = d * (unsigned)nbins + ((w >> (8 * (d & 3u))) & 0xffu);
+      if (dim >= 11) {  // three turns, unrolled
+#pragma unroll
+        for (unsigned t = 0; t < 3; ++t) {
+          if (ok && turn == t) wh[cell] += h2[p];
+          __syncwarp();
+        }
+      } else {
+#pragma unroll 1
+        for (unsigned t = 0; t * (unsigned)dim < 32u; ++t) {
+          if (ok && turn == t) wh[cell] += h2[p];
+          __syncwarp();
+        }
       }
       d = d + 1u == (unsigned)dim ? 0u : d + 1u;
     }
