@@ -194,6 +194,28 @@ int fiesta_estimate_from_sums(fiesta_ctx *ctx, const fiesta_program *prog, const
                               int32_t n_shifts, uint64_t n_per_shift, const double *sums_host,
                               const uint64_t *nonfinite_host, fiesta_result *out);
 
+/* ---- no device allocation (for callers that cannot call cudaMalloc) ----------------------------
+ *
+ * The per-shift sums of fiesta_partial_sums for ONE real sector under the lattice or the plain-MC
+ * rule, computed without cudaMalloc, cudaFree or any allocating library routine: the partial records
+ * live in a file-scope device array of fixed size that every GPU holds from the moment it loads
+ * the library until the process exits (1 MiB + 256 B: 4096 records).  Limit: n_shifts x chunks <=
+ * 4096 -- a chunk is at most 2^17 points, so up to 2^29 points per call; beyond it the call fails
+ * with FIESTA_E_TOOBIG before anything is launched.  Vegas: FIESTA_E_RULE; complex sector:
+ * FIESTA_E_ARG.  The evaluation runs on the interpreter kernel in plain FP64 (fiesta_set_mixed is
+ * ignored), with the chunking and the order of additions of fiesta_partial_sums: the same bits.
+ *
+ * sums_dev: DEVICE memory of the caller, [n_shifts][K][2] doubles (S1, S2; n_shifts = 1 for MC);
+ * nonfinite_dev: DEVICE memory, one uint64 (count of NaN / Inf values), or NULL.  The work is queued
+ * on the context's stream and the call returns without waiting (_async): synchronise that stream
+ * before reading.  The first call on a device resolves the array's address, which may load this
+ * part of the library's device code: make one warm-up call before a region that must not allocate.
+ * All calls on a device share the array: calls that overlap on the GPU (other streams or contexts)
+ * race -- serialise them. */
+int fiesta_partial_sums_noalloc_async(fiesta_ctx *ctx, const fiesta_program *prog, int32_t sector, int32_t dim,
+                                      uint64_t npoints, const fiesta_rule *rule, uint64_t seed, double *sums_dev,
+                                      uint64_t *nonfinite_dev);
+
 /* ---- deterministic integrator (PAPER.md:412 `CurrentIntegrator -> cuhreCuba`) ------
  *
  * A Cuhre-like globally adaptive cubature on the same evaluator (R21): the degree-7 rule of

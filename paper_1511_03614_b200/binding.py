@@ -91,6 +91,7 @@ _SIGNATURES = {
     "fiesta_partial_sums_shifts": (C.c_int, [_VP, _VP, _VP, _I32, _I32, _U64, C.POINTER(_Rule), _U64, _I32, _I32, _I32, _VP]),
     "fiesta_last_nonfinite": (C.c_int, [_VP, _I32, _VP]),
     "fiesta_estimate_from_sums": (C.c_int, [_VP, _VP, _VP, _I32, _I32, _U64, _VP, _VP, _VP]),
+    "fiesta_partial_sums_noalloc_async": (C.c_int, [_VP, _VP, _I32, _I32, _U64, C.POINTER(_Rule), _U64, _VP, _VP]),
     "fiesta_set_mixed": (C.c_int, [_VP, C.c_double]),
     "fiesta_eval_points_dd": (C.c_int, [_VP, _VP, _I32, _VP, _U64, _VP]),
 }
@@ -331,6 +332,14 @@ class Context:
         self._check(self.lib.fiesta_cubature_rule(self.handle, prog.handle, int(sector), int(tier), _ptr(boxes), nb, _ptr(i7),
                                                   _ptr(i5), _ptr(fourth), _ptr(axis)))
         return i7[..., 0] + 1j * i7[..., 1], i5[..., 0] + 1j * i5[..., 1], fourth, axis
+
+    def partial_sums_noalloc_async(self, prog, sector, npoints, rule, seed, sums_dev, nonfinite_dev=0):
+        """fiesta_partial_sums_noalloc_async: sums_dev / nonfinite_dev are raw DEVICE addresses (integers, e.g.
+        tensor.data_ptr()) of [R][K][2] doubles and one uint64; queued on the context's stream, no synchronisation."""
+        r, keep = rule._c()
+        self._check(self.lib.fiesta_partial_sums_noalloc_async(self.handle, prog.handle, int(sector), prog.dim, int(npoints),
+                                                               C.byref(r), int(seed), _VP(int(sums_dev)),
+                                                               _VP(int(nonfinite_dev)) if nonfinite_dev else None))
 
     def set_mixed(self, small_x):
         """Mixed precision: points with min_k x_k < small_x are evaluated in double-double (0: off)."""

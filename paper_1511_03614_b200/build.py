@@ -123,6 +123,7 @@ def build(force=False, verbose=False):
     cu("fx_kernels_small", "fx_kernels_small.cu")
     cu("fx_kernels_dd", "fx_kernels_dd.cu")
     cu("fx_kernels_cubature", "fx_kernels_cubature.cu")
+    cu("fx_kernels_noalloc", "fx_kernels_noalloc.cu")
     for n in CPLX_DIMS:
         cu("fx_kernels_cplx_n%d" % n, "fx_kernels_cplx.cu", ["-DFX_N=%d" % n])
     for name in ("fiesta_abi", "fx_compiler", "fx_jit"):

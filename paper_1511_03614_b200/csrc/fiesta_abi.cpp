@@ -672,6 +672,7 @@ int fiesta_combine(const fiesta_result *per_sector, int32_t nsectors, int32_t K,
 // ------------------------------------------------------------------------------------------------
 #include "fiesta_abi_integrate.inc"
 #include "fiesta_abi_cubature.inc"
+#include "fiesta_abi_noalloc.inc"
 
 // ------------------------------------------------------------------------------------------------
 // dispatch of the complex kernels, one translation unit per dimension (fx_kernels_cplx.cu -DFX_N=n)
