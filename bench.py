@@ -275,7 +275,7 @@ class Timer:
 # dram__bytes_read.sum + dram__bytes_write.sum of one native-kernel launch, from the committed ncu --set full
 # captures (profiles/r02_ncu_fxj_integrate_c3.md, _c4.md, _c5.md): the points are made on the device and a block
 # writes one 256-byte record, so the traffic of the ALU-bound kernels is the program text and the parameters
-NCU_DRAM_BYTES = {"C3": 56832, "C4": 54784, "C5": 38656}
+NCU_DRAM_BYTES = {"C3": 56832, "C4": 54784, "C5": 37888}
 
 
 def roofline_of(wl, prog, S, kern_ms, peak_live, tiers):
