@@ -248,3 +248,18 @@ def test_native_assemble_rejects_bad_input(lib):
     with pytest.raises(lib.FiestaError) as e:
         lib.native_assemble(SectorText(sector_id=0, texts=["1;\n0;\nx[1]+;\n|"]), 1)
     assert "line" in str(e.value) or "expected" in str(e.value) or len(str(e.value)) > 0
+
+
+def test_no_alloc_entry_point_sources_call_no_allocator():
+    """fiesta_partial_sums_noalloc_async (fx_kernels_noalloc.cu, fiesta_abi_noalloc.inc): no device allocation call in
+    its own code (comments aside), a static scratch array with a stated size, and the address from cudaGetSymbolAddress."""
+    csrc = os.path.join(ROOT, "paper_1511_03614_b200", "csrc")
+    code = ""
+    for name in ("fx_kernels_noalloc.cu", "fiesta_abi_noalloc.inc"):
+        text = open(os.path.join(csrc, name)).read()
+        code += re.sub(r"//[^\n]*", "", text)
+    for banned in ("cudaMalloc", "cudaFree", "cudaMallocAsync", "cudaHostAlloc", "cuMemAlloc", "reserve("):
+        assert banned not in code, banned
+    assert "static __device__ __align__(256) double fx_noalloc_scratch[" in code
+    assert "cudaGetSymbolAddress(&p, fx_noalloc_scratch)" in code
+    assert re.search(r"#define FX_NOALLOC_MAX_BLOCKS 4096\b", code)
