@@ -13,7 +13,8 @@ struct fx_smem_layout {
   uint32_t prog, mem, acc, delta, tf, grid, hist, wsum, total;
 };
 
-__host__ __device__ inline fx_smem_layout fx_layout(int prog_ins, int mem_doubles, int dim, int nbins, bool vegas) {
+__host__ __device__ inline fx_smem_layout fx_layout(int prog_ins, int mem_doubles, int dim, int nbins, bool vegas,
+                                                    int acc_slots = FX_ACC_SLOTS) {
   fx_smem_layout L;
   uint32_t o = 0;
   L.prog = o;
@@ -21,7 +22,7 @@ __host__ __device__ inline fx_smem_layout fx_layout(int prog_ins, int mem_double
   L.mem = o;
   o += (uint32_t)mem_doubles * 8u;
   L.acc = o;
-  o += FX_ACC_SLOTS * FX_THREADS * 8u;
+  o += (uint32_t)acc_slots * FX_THREADS * 8u;
   L.delta = o;
   o += FX_NXMAX * 8u;
   L.tf = o;

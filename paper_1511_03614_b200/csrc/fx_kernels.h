@@ -74,6 +74,8 @@ struct fx_integrate_params {
   // here and evaluated in double-double by fx_launch_rescue_real.  0: off.
   double small_x;
   int32_t shift_base;        // lattice: the block's shift r stands for shift shift_base + r of the rule (a rank's share of the shifts)
+  int32_t acc_slots_real;    // accumulator slots per thread the real interpreter kernel reserves in shared memory: 2 K of the
+                             // call's real sectors + FX_P_REAL + 1 (0: FX_ACC_SLOTS).  Less shared memory per block = one more resident block.
 };
 
 // position in the selection of the sector a block works on

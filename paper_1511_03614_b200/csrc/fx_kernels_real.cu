@@ -7,17 +7,24 @@
 
 namespace {
 
+// accumulator slots of a launch: what the call's real sectors need (make_plan), not the record's 32
+// (2 K_max accumulators + FX_P_REAL weights + 1 counter: fiesta_abi_integrate.inc make_plan)
+__host__ __device__ inline int fx_real_acc_slots(const fx_integrate_params &prm) {
+  return prm.acc_slots_real > 0 ? prm.acc_slots_real : FX_ACC_SLOTS;
+}
+
 template <int P>
 struct IntegrateSinkReal {
-  double *acc;  // &acc[0][tid], slot stride FX_THREADS
-  const double (&W)[P];
+  double *acc;      // &acc[0][tid], slot stride FX_THREADS
+  const double *W;  // &W[0][tid] in shared memory, stride FX_THREADS: read here, at the outputs, instead of held in
+                    // 2 P registers across the walk (that is what lets 4 blocks of 128 registers be resident)
   unsigned valid;
   unsigned nonfinite;
   double (&h2)[P];
   __device__ __forceinline__ void operator()(int k, double (&A)[P]) {
     double s1 = acc[(2 * k) * FX_THREADS], s2 = acc[(2 * k + 1) * FX_THREADS];
     FX_PLOOP {
-      double g = W[p] * A[p];
+      double g = W[p * FX_THREADS] * A[p];
       if (!((valid >> p) & 1u)) g = 0.0;
       nonfinite += isfinite(g) ? 0u : 1u;
       s1 += g;
@@ -30,7 +37,7 @@ struct IntegrateSinkReal {
 };
 
 template <int NX, int RULE>
-__global__ void __launch_bounds__(FX_THREADS, NX <= 4 ? 4 : NX <= 8 ? 3 : 2) fx_integrate_real(const __grid_constant__ fx_integrate_params prm) {
+__global__ void __launch_bounds__(FX_THREADS, NX <= 4 ? 4 : NX <= 8 ? (RULE == FIESTA_RULE_LATTICE ? 4 : 3) : (RULE == FIESTA_RULE_LATTICE ? 3 : 2)) fx_integrate_real(const __grid_constant__ fx_integrate_params prm) {
   constexpr int P = FX_P_REAL;
   extern __shared__ __align__(16) unsigned char smem[];
   const int b = blockIdx.x;
@@ -40,7 +47,7 @@ __global__ void __launch_bounds__(FX_THREADS, NX <= 4 ? 4 : NX <= 8 ? 3 : 2) fx_
   const fx_sector_dev sec = prm.sectors[prm.sel[sel_idx]];
   const int dim = prm.dim;
   constexpr bool vegas = RULE == FIESTA_RULE_VEGAS;
-  const fx_smem_layout L = fx_layout(prm.prog_ins_max, prm.mem_doubles, dim, prm.nbins, vegas);
+  const fx_smem_layout L = fx_layout(prm.prog_ins_max, prm.mem_doubles, dim, prm.nbins, vegas, fx_real_acc_slots(prm));
   fx_ins *sh_prog = reinterpret_cast<fx_ins *>(smem + L.prog);
   double *sh_mem = reinterpret_cast<double *>(smem + L.mem);
   double *sh_acc = reinterpret_cast<double *>(smem + L.acc);
@@ -53,12 +60,15 @@ __global__ void __launch_bounds__(FX_THREADS, NX <= 4 ? 4 : NX <= 8 ? 3 : 2) fx_
   fx_block_setup(prm, dim, (uint32_t)sec.sector_id, r, sel_idx, sh_delta, sh_grid, sh_hist);
   const int nslots = 2 * sec.K;
   for (int s = 0; s < nslots; ++s) sh_acc[s * FX_THREADS + threadIdx.x] = 0.0;
+  // behind the accumulators: this thread's P weights and its count of non-finite values
+  double *sh_w = sh_acc + (size_t)(fx_real_acc_slots(prm) - (P + 1)) * FX_THREADS + threadIdx.x;
+  unsigned *sh_nf = reinterpret_cast<unsigned *>(sh_w + P * FX_THREADS);
+  *sh_nf = 0u;
   __syncthreads();
 
   const uint64_t c0 = (uint64_t)chunk * prm.chunk;
   const uint64_t c1 = min(c0 + prm.chunk, prm.n_per_shift);
   const fx_mem<double> M{sh_mem + threadIdx.x, FX_THREADS};
-  unsigned nonfinite = 0;
   // the trip count is the same for every thread of the block (points past the end are masked by
   // `valid`): the Vegas histogram update is a warp-collective operation
   for (uint64_t it = c0; it < c1; it += (uint64_t)FX_THREADS * P) {
@@ -67,15 +77,20 @@ __global__ void __launch_bounds__(FX_THREADS, NX <= 4 ? 4 : NX <= 8 ? 3 : 2) fx_
     uint32_t bins[(NX + 3) / 4][P];
     unsigned valid;
     fx_make_points<RULE, NX, P, RULE == FIESTA_RULE_VEGAS>(prm, dim, (uint32_t)sec.sector_id, sh_delta, sh_grid, base, c1, x, xbar, W, valid, bins);
-    FX_PLOOP { h2[p] = 0.0; }
-    IntegrateSinkReal<P> sink{sh_acc + threadIdx.x, W, valid, 0u, h2};
+    FX_PLOOP {
+      h2[p] = 0.0;
+      sh_w[p * FX_THREADS] = W[p];
+    }
+    IntegrateSinkReal<P> sink{sh_acc + threadIdx.x, sh_w, valid, 0u, h2};
     fx_run<double, NX, P>(sh_prog, x, M, sink);
-    nonfinite += sink.nonfinite;
+    *sh_nf += sink.nonfinite;
     if (vegas) fx_hist_points<NX, P>(sh_hist, dim, prm.nbins, valid, bins, h2);
   }
   __syncthreads();
-  fx_block_reduce(sh_acc, sh_wsum, nslots, fx_partial_record(prm, sel_idx, r, chunk));
-  fx_block_finish(prm, dim, sel_idx, chunk, nonfinite, sh_hist);
+  const unsigned nonfinite = *sh_nf;
+  const fx_block_id id1 = fx_block_coords(prm);  // computed again (volatile read of the block index) rather than kept across the walk
+  fx_block_reduce(sh_acc, sh_wsum, 2 * prm.sectors[prm.sel[id1.sel_idx]].K, fx_partial_record(prm, id1.sel_idx, id1.r, id1.chunk));
+  fx_block_finish(prm, prm.dim, id1.sel_idx, id1.chunk, nonfinite, sh_hist);
 }
 
 template <int P>
@@ -129,7 +144,8 @@ size_t fx_integrate_smem_bytes(const fx_integrate_params &prm) {
 }
 
 cudaError_t fx_launch_integrate_real(const fx_integrate_params &prm, int nsectors, cudaStream_t st) {
-  const size_t smem = fx_integrate_smem_bytes(prm);
+  const size_t smem = fx_layout(prm.prog_ins_max, prm.mem_doubles, prm.dim, prm.nbins, prm.rule == FIESTA_RULE_VEGAS,
+                                fx_real_acc_slots(prm)).total;
   const unsigned grid = (unsigned)((size_t)nsectors * prm.n_shifts * prm.nchunks);
   cudaError_t e;
 #define FX_LAUNCH2(NX, RULE)                                                            \
