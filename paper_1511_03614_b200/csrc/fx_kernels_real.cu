@@ -73,6 +73,7 @@ __global__ void __launch_bounds__(FX_THREADS, NX <= 4 ? 4 : NX <= 8 ? (RULE == F
   // `valid`): the Vegas histogram update is a warp-collective operation
   for (uint64_t it = c0; it < c1; it += (uint64_t)FX_THREADS * P) {
     const uint64_t base = it + (uint64_t)threadIdx.x * P;
+    __syncthreads();  // the block's warps walk the program in step: one instruction stream through the caches
     double x[NX][P], xbar[NX][P], W[P], h2[P];
     uint32_t bins[(NX + 3) / 4][P];
     unsigned valid;
