@@ -688,7 +688,7 @@ size_t fx_eval_cplx_smem_bytes(const fx_eval_params &prm) {
 }
 
 cudaError_t fx_launch_integrate_cplx(const fx_integrate_params &prm, int nsectors, cudaStream_t st) {
-  const size_t smem = fx_integrate_smem_bytes(prm);
+  const size_t smem = fx_integrate_cplx_smem_bytes(prm);
   switch (prm.dim) {
 #define FX_CASE(n) case n: return fx_launch_integrate_cplx_n##n(prm, nsectors, smem, st);
     FX_CASE(1) FX_CASE(2) FX_CASE(3) FX_CASE(4) FX_CASE(5) FX_CASE(6) FX_CASE(7) FX_CASE(8)

@@ -76,6 +76,7 @@ struct fx_integrate_params {
   int32_t shift_base;        // lattice: the block's shift r stands for shift shift_base + r of the rule (a rank's share of the shifts)
   int32_t acc_slots_real;    // accumulator slots per thread the real interpreter kernel reserves in shared memory: 2 K of the
                              // call's real sectors + FX_P_REAL + 1 (0: FX_ACC_SLOTS).  Less shared memory per block = one more resident block.
+  int32_t acc_slots_cplx;    // the same for the complex interpreter kernel: 4 K of the call's complex sectors (0: FX_ACC_SLOTS)
 };
 
 // position in the selection of the sector a block works on
@@ -96,6 +97,7 @@ struct fx_eval_params {
 };
 
 size_t fx_integrate_smem_bytes(const fx_integrate_params &p);
+size_t fx_integrate_cplx_smem_bytes(const fx_integrate_params &p);  // fx_integrate_cplx: accumulator area sized by acc_slots_cplx
 
 // Shared-memory layout of the native kernels (fx_jit_template*.cu): accumulators (sum g, sum g^2 per
 // output component: FXJ_ACC_SLOTS slots, one column per thread), the lattice shifts, the transform

@@ -56,13 +56,17 @@ __device__ __forceinline__ void fx_deform_points(const fx_ins *sh_deform, double
     const cplx d = fx_jacobian_det<N>(lambda, xv, xbv, [&](int slot) { return M.ld(slot, p, P); }, zi);
 #pragma unroll
     for (int k = 0; k < N; ++k) M.st(k, p, P, zi[k]);
-    M.st(NGH + 2 * N, p, P, d.re);
-    M.st(NGH + 2 * N + 1, p, P, d.im);
+    if constexpr (P == 1) {
+      det[0] = d;  // the elimination is over: its result stays in registers
+    } else {
+      M.st(NGH + 2 * N, p, P, d.re);
+      M.st(NGH + 2 * N + 1, p, P, d.im);
+    }
   }
   // x is re-read from its slot: nothing but J has to stay in registers across the elimination
 #pragma unroll
   for (int k = 0; k < N; ++k) FX_PLOOP { X[k][p] = cplx{M.ld(NGH + k, p, P), M.ld(k, p, P)}; }
-  FX_PLOOP { det[p] = cplx{M.ld(NGH + 2 * N, p, P), M.ld(NGH + 2 * N + 1, p, P)}; }
+  if constexpr (P != 1) FX_PLOOP { det[p] = cplx{M.ld(NGH + 2 * N, p, P), M.ld(NGH + 2 * N + 1, p, P)}; }
 }
 
 struct IntegrateSinkCplx {
@@ -100,7 +104,9 @@ __global__ void __launch_bounds__(FX_THREADS) fx_integrate_cplx(const __grid_con
   const int sel_idx = fx_sel_index(prm, b / (prm.nchunks * prm.n_shifts));
   const fx_sector_dev sec = prm.sectors[prm.sel[sel_idx]];
   constexpr bool vegas = RULE == FIESTA_RULE_VEGAS;
-  const fx_smem_layout L = fx_layout(prm.prog_ins_max, prm.mem_doubles, N, prm.nbins, vegas);
+  // the accumulator area holds what the call's complex sectors need (4 K slots), not the record's 32: one more resident block
+  const fx_smem_layout L = fx_layout(prm.prog_ins_max, prm.mem_doubles, N, prm.nbins, vegas,
+                                     prm.acc_slots_cplx > 0 ? prm.acc_slots_cplx : FX_ACC_SLOTS);
   fx_ins *sh_prog = reinterpret_cast<fx_ins *>(smem + L.prog);
   fx_ins *sh_deform = sec.deform_len ? sh_prog + sec.main_len : nullptr;
   double *sh_mem = reinterpret_cast<double *>(smem + L.mem);

@@ -140,6 +140,11 @@ cudaError_t set_smem(K kernel, size_t bytes) {
 
 }  // namespace
 
+size_t fx_integrate_cplx_smem_bytes(const fx_integrate_params &prm) {
+  return fx_layout(prm.prog_ins_max, prm.mem_doubles, prm.dim, prm.nbins, prm.rule == FIESTA_RULE_VEGAS,
+                   prm.acc_slots_cplx > 0 ? prm.acc_slots_cplx : FX_ACC_SLOTS).total;
+}
+
 size_t fx_integrate_smem_bytes(const fx_integrate_params &prm) {
   return fx_layout(prm.prog_ins_max, prm.mem_doubles, prm.dim, prm.nbins, prm.rule == FIESTA_RULE_VEGAS).total;
 }
