@@ -37,7 +37,7 @@ struct IntegrateSinkReal {
 };
 
 template <int NX, int RULE>
-__global__ void __launch_bounds__(FX_THREADS, NX <= 4 ? 4 : NX <= 8 ? (RULE == FIESTA_RULE_LATTICE ? 4 : 3) : (RULE == FIESTA_RULE_LATTICE ? 3 : 2)) fx_integrate_real(const __grid_constant__ fx_integrate_params prm) {
+__global__ void __launch_bounds__(FX_THREADS, NX <= 4 ? 4 : NX <= 8 ? (RULE == FIESTA_RULE_LATTICE ? 4 : 3) : (RULE == FIESTA_RULE_VEGAS ? 2 : 3)) fx_integrate_real(const __grid_constant__ fx_integrate_params prm) {
   constexpr int P = FX_P_REAL;
   extern __shared__ __align__(16) unsigned char smem[];
   const int b = blockIdx.x;
