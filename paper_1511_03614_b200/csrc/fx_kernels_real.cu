@@ -13,14 +13,14 @@ __host__ __device__ inline int fx_real_acc_slots(const fx_integrate_params &prm)
   return prm.acc_slots_real > 0 ? prm.acc_slots_real : FX_ACC_SLOTS;
 }
 
-template <int P>
+template <int P, bool VEGAS>
 struct IntegrateSinkReal {
   double *acc;      // &acc[0][tid], slot stride FX_THREADS
   const double *W;  // &W[0][tid] in shared memory, stride FX_THREADS: read here, at the outputs, instead of held in
                     // 2 P registers across the walk (that is what lets 4 blocks of 128 registers be resident)
   unsigned valid;
   unsigned nonfinite;
-  double (&h2)[P];
+  double *h2;       // Vegas: &h2[0][tid] in shared memory (sum over the orders of g^2, for the histogram)
   __device__ __forceinline__ void operator()(int k, double (&A)[P]) {
     double s1 = acc[(2 * k) * FX_THREADS], s2 = acc[(2 * k + 1) * FX_THREADS];
     FX_PLOOP {
@@ -29,7 +29,7 @@ struct IntegrateSinkReal {
       nonfinite += isfinite(g) ? 0u : 1u;
       s1 += g;
       s2 = fma(g, g, s2);
-      h2[p] = fma(g, g, h2[p]);
+      if constexpr (VEGAS) h2[p * FX_THREADS] = fma(g, g, h2[p * FX_THREADS]);
     }
     acc[(2 * k) * FX_THREADS] = s1;
     acc[(2 * k + 1) * FX_THREADS] = s2;
@@ -37,7 +37,7 @@ struct IntegrateSinkReal {
 };
 
 template <int NX, int RULE>
-__global__ void __launch_bounds__(FX_THREADS, NX <= 4 ? 4 : NX <= 8 ? (RULE == FIESTA_RULE_LATTICE ? 4 : 3) : (RULE == FIESTA_RULE_VEGAS ? 2 : 3)) fx_integrate_real(const __grid_constant__ fx_integrate_params prm) {
+__global__ void __launch_bounds__(FX_THREADS, NX <= 4 ? 4 : NX <= 8 ? (RULE == FIESTA_RULE_LATTICE ? 4 : 3) : 3) fx_integrate_real(const __grid_constant__ fx_integrate_params prm) {
   constexpr int P = FX_P_REAL;
   extern __shared__ __align__(16) unsigned char smem[];
   const int b = blockIdx.x;
@@ -60,9 +60,14 @@ __global__ void __launch_bounds__(FX_THREADS, NX <= 4 ? 4 : NX <= 8 ? (RULE == F
   fx_block_setup(prm, dim, (uint32_t)sec.sector_id, r, sel_idx, sh_delta, sh_grid, sh_hist);
   const int nslots = 2 * sec.K;
   for (int s = 0; s < nslots; ++s) sh_acc[s * FX_THREADS + threadIdx.x] = 0.0;
-  // behind the accumulators: this thread's P weights and its count of non-finite values
-  double *sh_w = sh_acc + (size_t)(fx_real_acc_slots(prm) - (P + 1)) * FX_THREADS + threadIdx.x;
+  // behind the accumulators: this thread's P weights and its count of non-finite values; for Vegas also the
+  // points' sums of g^2 and their bins, which are needed only after the walk
+  constexpr int NBW = (NX + 3) / 4;                       // 32-bit words of bins per point
+  constexpr int XTRA = vegas ? P + (NBW * P + 1) / 2 : 0;  // doubles per thread (make_plan reserves them)
+  double *sh_w = sh_acc + (size_t)(fx_real_acc_slots(prm) - (P + 1 + XTRA)) * FX_THREADS + threadIdx.x;
   unsigned *sh_nf = reinterpret_cast<unsigned *>(sh_w + P * FX_THREADS);
+  double *sh_h2 = sh_w + (P + 1) * FX_THREADS;
+  uint32_t *sh_bins = reinterpret_cast<uint32_t *>(sh_acc + (size_t)(fx_real_acc_slots(prm) - (NBW * P + 1) / 2) * FX_THREADS) + threadIdx.x;
   *sh_nf = 0u;
   __syncthreads();
 
@@ -74,18 +79,33 @@ __global__ void __launch_bounds__(FX_THREADS, NX <= 4 ? 4 : NX <= 8 ? (RULE == F
   for (uint64_t it = c0; it < c1; it += (uint64_t)FX_THREADS * P) {
     const uint64_t base = it + (uint64_t)threadIdx.x * P;
     __syncthreads();  // the block's warps walk the program in step: one instruction stream through the caches
-    double x[NX][P], xbar[NX][P], W[P], h2[P];
-    uint32_t bins[(NX + 3) / 4][P];
+    double x[NX][P], xbar[NX][P], W[P];
     unsigned valid;
-    fx_make_points<RULE, NX, P, RULE == FIESTA_RULE_VEGAS>(prm, dim, (uint32_t)sec.sector_id, sh_delta, sh_grid, base, c1, x, xbar, W, valid, bins);
-    FX_PLOOP {
-      h2[p] = 0.0;
-      sh_w[p * FX_THREADS] = W[p];
+    {
+      uint32_t bins[NBW][P];
+      fx_make_points<RULE, NX, P, RULE == FIESTA_RULE_VEGAS>(prm, dim, (uint32_t)sec.sector_id, sh_delta, sh_grid, base, c1, x, xbar, W, valid, bins);
+      FX_PLOOP {
+        sh_w[p * FX_THREADS] = W[p];
+        if constexpr (vegas) {
+          sh_h2[p * FX_THREADS] = 0.0;
+#pragma unroll
+          for (int q = 0; q < NBW; ++q) sh_bins[(q * P + p) * FX_THREADS] = bins[q][p];
+        }
+      }
     }
-    IntegrateSinkReal<P> sink{sh_acc + threadIdx.x, sh_w, valid, 0u, h2};
+    IntegrateSinkReal<P, vegas> sink{sh_acc + threadIdx.x, sh_w, valid, 0u, sh_h2};
     fx_run<double, NX, P>(sh_prog, x, M, sink);
     *sh_nf += sink.nonfinite;
-    if (vegas) fx_hist_points<NX, P>(sh_hist, dim, prm.nbins, valid, bins, h2);
+    if constexpr (vegas) {
+      uint32_t bins[NBW][P];
+      double h2[P];
+      FX_PLOOP {
+        h2[p] = sh_h2[p * FX_THREADS];
+#pragma unroll
+        for (int q = 0; q < NBW; ++q) bins[q][p] = sh_bins[(q * P + p) * FX_THREADS];
+      }
+      fx_hist_points<NX, P>(sh_hist, dim, prm.nbins, valid, bins, h2);
+    }
   }
   __syncthreads();
   const unsigned nonfinite = *sh_nf;
